@@ -1,0 +1,210 @@
+"""ctypes binding of include/lgf.h (argument marshalling only; every step runs in the CUDA kernels)."""
+from __future__ import annotations
+
+import ctypes
+import os
+import re
+from dataclasses import dataclass
+from typing import Optional, Sequence
+
+LGF_F32, LGF_F64 = 0, 1
+LGF_REAL18, LGF_REAL12 = 18, 12
+LGF_HOST, LGF_DEVICE = 0, 1
+
+_HERE = os.path.dirname(os.path.abspath(__file__))
+_HEADER = os.path.join(os.path.dirname(_HERE), "include", "lgf.h")
+_lib: Optional[ctypes.CDLL] = None
+
+
+class LgfError(RuntimeError):
+    pass
+
+
+class _Result(ctypes.Structure):
+    _fields_ = [("iterations", ctypes.c_int64), ("theta", ctypes.c_double), ("F", ctypes.c_double),
+                ("converged", ctypes.c_int32)]
+
+
+@dataclass
+class LgfResult:
+    iterations: int
+    theta: float
+    F: float
+    converged: bool
+
+
+def library_path() -> str:
+    return os.path.join(_HERE, "liblgf.so")
+
+
+def declared_symbols() -> list:
+    """Every function include/lgf.h declares (used by the CPU test that the library exports them)."""
+    text = open(_HEADER).read()
+    text = re.sub(r"/\*.*?\*/", "", text, flags=re.S)
+    return sorted(set(re.findall(r"\b(lgf_[a-z_0-9]+)\s*\(", text)))
+
+
+def load_library() -> ctypes.CDLL:
+    """dlopen liblgf.so (no build here: `__graft_entry__.build()` / `_build.build()` compile it)."""
+    global _lib
+    if _lib is not None:
+        return _lib
+    path = library_path()
+    if not os.path.exists(path):
+        raise LgfError(f"{path} is missing: run `python -m paper_1208_1186_b200._build` (there is no CPU fallback)")
+    lib = ctypes.CDLL(path)
+    i32p = ctypes.POINTER(ctypes.c_int32)
+    rp = ctypes.POINTER(_Result)
+    vp = ctypes.c_void_p
+    lib.lgf_workspace_bytes.restype = ctypes.c_size_t
+    lib.lgf_workspace_bytes.argtypes = [i32p, ctypes.c_int, ctypes.c_int]
+    lib.lgf_create.argtypes = [i32p, ctypes.c_int, ctypes.c_int, vp, ctypes.c_size_t, vp, ctypes.POINTER(vp)]
+    lib.lgf_create_simple.argtypes = [i32p, ctypes.c_int, ctypes.c_int, ctypes.POINTER(vp)]
+    lib.lgf_destroy.argtypes = [vp]
+    lib.lgf_load.argtypes = [vp, vp, ctypes.c_int]
+    lib.lgf_store.argtypes = [vp, vp, ctypes.c_int]
+    lib.lgf_measure.argtypes = [vp, rp]
+    lib.lgf_iterate.argtypes = [vp, ctypes.c_int64, ctypes.c_double, rp]
+    lib.lgf_iterate_async.argtypes = [vp, ctypes.c_int64, ctypes.c_double]
+    lib.lgf_wait.argtypes = [vp, rp]
+    lib.lgf_fix.argtypes = [vp, ctypes.c_double, ctypes.c_double, ctypes.c_int64, rp]
+    lib.lgf_profile_iterate.argtypes = [vp, ctypes.c_int64, ctypes.c_double, ctypes.POINTER(ctypes.c_double), rp]
+    lib.lgf_debug_get_delta.argtypes = [vp, vp, ctypes.c_int]
+    lib.lgf_debug_fourier_accelerate.argtypes = [vp]
+    lib.lgf_launch_count.restype = ctypes.c_int64
+    lib.lgf_launch_count.argtypes = [vp]
+    for f in (lib.lgf_strerror, lib.lgf_last_error, lib.lgf_version):
+        f.restype = ctypes.c_char_p
+    lib.lgf_strerror.argtypes = [ctypes.c_int]
+    _lib = lib
+    return lib
+
+
+def _L(L: Sequence[int]):
+    return (ctypes.c_int32 * 4)(*[int(v) for v in L])
+
+
+def workspace_bytes(L: Sequence[int], precision: int, storage: int) -> int:
+    return int(load_library().lgf_workspace_bytes(_L(L), precision, storage))
+
+
+def _check(rc: int, what: str) -> None:
+    if rc != 0:
+        lib = load_library()
+        raise LgfError(f"{what}: {lib.lgf_strerror(rc).decode()} [{rc}] {lib.lgf_last_error().decode()}")
+
+
+class GaugeFixer:
+    """One lattice on one GPU.  Methods mirror the C ABI: load, store, measure, iterate, fix."""
+
+    def __init__(self, L: Sequence[int], precision: int = LGF_F64, storage: int = LGF_REAL18,
+                 device: str = "cuda:0", stream=None):
+        import torch
+        if not torch.cuda.is_available():
+            raise LgfError("no CUDA device: the lgf library has no CPU fallback")
+        self._torch = torch
+        self.lib = load_library()
+        self.L = tuple(int(v) for v in L)
+        self.V = self.L[0] * self.L[1] * self.L[2] * self.L[3]
+        self.precision, self.storage = precision, storage
+        self.dtype = torch.float64 if precision == LGF_F64 else torch.float32
+        self.device = torch.device(device)
+        nbytes = self.lib.lgf_workspace_bytes(_L(self.L), precision, storage)
+        if nbytes == 0:
+            raise LgfError(f"unsupported lattice {self.L} (extents must be 2^a 3^b >= 2)")
+        with torch.cuda.device(self.device):
+            self.workspace = torch.empty(nbytes + 256, dtype=torch.uint8, device=self.device)
+            ptr = (self.workspace.data_ptr() + 255) // 256 * 256
+            self.stream = stream if stream is not None else torch.cuda.current_stream(self.device)
+            h = ctypes.c_void_p()
+            _check(self.lib.lgf_create(_L(self.L), precision, storage, ctypes.c_void_p(ptr), nbytes,
+                                       ctypes.c_void_p(self.stream.cuda_stream), ctypes.byref(h)), "lgf_create")
+        self._h = h
+
+    def close(self) -> None:
+        if getattr(self, "_h", None):
+            self.lib.lgf_destroy(self._h)
+            self._h = None
+
+    def __del__(self):
+        try:
+            self.close()
+        except Exception:
+            pass
+
+    # -- marshalling helpers
+    def _ptr_space(self, t):
+        assert t.dtype == self.dtype and t.is_contiguous(), (t.dtype, self.dtype)
+        return ctypes.c_void_p(t.data_ptr()), (LGF_DEVICE if t.is_cuda else LGF_HOST)
+
+    def load(self, links) -> None:
+        """links: real tensor [V,4,3,3,2] (host or device) of the context precision."""
+        assert links.numel() == self.V * 72
+        p, sp = self._ptr_space(links)
+        with self._torch.cuda.device(self.device):
+            _check(self.lib.lgf_load(self._h, p, sp), "lgf_load")
+
+    def store(self, out=None, device=None):
+        torch = self._torch
+        if out is None:
+            out = torch.empty(self.V, 4, 3, 3, 2, dtype=self.dtype, device=device or "cpu")
+        p, sp = self._ptr_space(out)
+        with torch.cuda.device(self.device):
+            _check(self.lib.lgf_store(self._h, p, sp), "lgf_store")
+        return out
+
+    @staticmethod
+    def _res(r: _Result) -> LgfResult:
+        return LgfResult(int(r.iterations), float(r.theta), float(r.F), bool(r.converged))
+
+    def measure(self) -> LgfResult:
+        r = _Result()
+        with self._torch.cuda.device(self.device):
+            _check(self.lib.lgf_measure(self._h, ctypes.byref(r)), "lgf_measure")
+        return self._res(r)
+
+    def iterate(self, n: int, alpha: float) -> LgfResult:
+        r = _Result()
+        with self._torch.cuda.device(self.device):
+            _check(self.lib.lgf_iterate(self._h, int(n), float(alpha), ctypes.byref(r)), "lgf_iterate")
+        return self._res(r)
+
+    def iterate_async(self, n: int, alpha: float) -> None:
+        with self._torch.cuda.device(self.device):
+            _check(self.lib.lgf_iterate_async(self._h, int(n), float(alpha)), "lgf_iterate_async")
+
+    def wait(self) -> LgfResult:
+        r = _Result()
+        with self._torch.cuda.device(self.device):
+            _check(self.lib.lgf_wait(self._h, ctypes.byref(r)), "lgf_wait")
+        return self._res(r)
+
+    def fix(self, alpha: float, theta_tol: float, max_iter: int) -> LgfResult:
+        r = _Result()
+        with self._torch.cuda.device(self.device):
+            _check(self.lib.lgf_fix(self._h, float(alpha), float(theta_tol), int(max_iter), ctypes.byref(r)), "lgf_fix")
+        return self._res(r)
+
+    KERNELS = ("K2_fft_xy_fwd", "K3_fft_zt_fwd_scale_inv", "K4_fft_xy_inv", "K5_gbuild_update", "K1_delta_theta_F")
+
+    def profile_iterate(self, n: int, alpha: float):
+        """-> (dict kernel name -> average ms per launch, LgfResult)."""
+        ms = (ctypes.c_double * 5)()
+        r = _Result()
+        with self._torch.cuda.device(self.device):
+            _check(self.lib.lgf_profile_iterate(self._h, int(n), float(alpha), ms, ctypes.byref(r)), "lgf_profile_iterate")
+        return {k: float(ms[i]) for i, k in enumerate(self.KERNELS)}, self._res(r)
+
+    def debug_delta(self):
+        """Packed Delta field as a host tensor [V,4,2]."""
+        out = self._torch.empty(self.V, 4, 2, dtype=self.dtype)
+        with self._torch.cuda.device(self.device):
+            _check(self.lib.lgf_debug_get_delta(self._h, ctypes.c_void_p(out.data_ptr()), LGF_HOST), "lgf_debug_get_delta")
+        return out
+
+    def debug_fourier_accelerate(self) -> None:
+        with self._torch.cuda.device(self.device):
+            _check(self.lib.lgf_debug_fourier_accelerate(self._h), "lgf_debug_fourier_accelerate")
+
+    def launch_count(self) -> int:
+        return int(self.lib.lgf_launch_count(self._h))

@@ -1,0 +1,670 @@
+// lgf_api.cu -- the C ABI of include/lgf.h: context, workspace carving, tables, launch plans,
+// CUDA-graph iteration body and the device-resident convergence loop (north_star subsystem (e)).
+// Product code (sm_100a); shares nothing with oracle/.  No CPU fallback anywhere: every compute
+// entry point launches kernels and reports LGF_ECUDA if that fails.
+#include "../../include/lgf.h"
+
+#include <cmath>
+#include <cstdio>
+#include <cstring>
+#include <new>
+#include <vector>
+
+#include "lgf_fft.cuh"
+#include "lgf_site.cuh"
+
+using namespace lgf;
+
+namespace {
+
+thread_local char g_last_error[512] = "";
+
+int cuda_fail(cudaError_t e, const char* what) {
+    snprintf(g_last_error, sizeof(g_last_error), "%s: %s", what, cudaGetErrorString(e));
+    return LGF_ECUDA;
+}
+#define CU(call)                                              \
+    do {                                                      \
+        cudaError_t e__ = (call);                             \
+        if (e__ != cudaSuccess) return cuda_fail(e__, #call); \
+    } while (0)
+
+constexpr size_t kAlign = 256;
+size_t align_up(size_t v) { return (v + kAlign - 1) / kAlign * kAlign; }
+
+typedef SiteTile<8, 4, 4, 2> TileA;
+constexpr int kStageSites = 1 << 15;       // boundary staging chunk (sites)
+constexpr int kMaxSmem = 200 * 1024;       // per-CTA dynamic shared memory we are willing to ask for
+constexpr int kFixBatch = 8;               // iterations enqueued per polling batch in lgf_fix
+
+bool factor23(int n, Axis* ax) {
+    if (n < 2) return false;
+    ax->N = n;
+    ax->nstages = 0;
+    ax->radices = 0;
+    int m = n;
+    auto push = [&](int r) { ax->radices |= (unsigned long long)r << (4 * ax->nstages); ax->nstages++; };
+    while (m % 8 == 0 && ax->nstages < kMaxStages) { push(8); m /= 8; }
+    while (m % 4 == 0 && ax->nstages < kMaxStages) { push(4); m /= 4; }
+    while (m % 2 == 0 && ax->nstages < kMaxStages) { push(2); m /= 2; }
+    while (m % 3 == 0 && ax->nstages < kMaxStages) { push(3); m /= 3; }
+    return m == 1;
+}
+
+struct Layout {          // byte offsets into the workspace
+    size_t state, partials, tw[4], twi[4], psq[4], links, delta, staging, total;
+    int nblocks_site;
+    int nb[4];
+};
+
+bool valid_args(const int32_t L[4], int precision, int storage) {
+    if (!L) return false;
+    if (precision != LGF_F32 && precision != LGF_F64) return false;
+    if (storage != LGF_REAL18 && storage != LGF_REAL12) return false;
+    for (int i = 0; i < 4; ++i)
+        if (L[i] < 2 || L[i] > 4096) return false;
+    return true;
+}
+
+Layout make_layout(const int32_t L[4], int precision, int storage) {
+    Layout lo;
+    const size_t w = precision == LGF_F64 ? 8 : 4;
+    const size_t V = (size_t)L[0] * L[1] * L[2] * L[3];
+    const int tile[4] = {8, 4, 4, 2};
+    size_t nb = 1;
+    for (int i = 0; i < 4; ++i) { lo.nb[i] = (L[i] + tile[i] - 1) / tile[i]; nb *= lo.nb[i]; }
+    lo.nblocks_site = (int)nb;
+    size_t off = 0;
+    lo.state = off; off += align_up(sizeof(DevState));
+    lo.partials = off; off += align_up(nb * sizeof(double2));
+    for (int i = 0; i < 4; ++i) { lo.tw[i] = off; off += align_up((size_t)L[i] * 2 * w); }
+    for (int i = 0; i < 4; ++i) { lo.twi[i] = off; off += align_up((size_t)L[i] * 2 * w); }
+    for (int i = 0; i < 4; ++i) { lo.psq[i] = off; off += align_up((size_t)L[i] * w); }
+    lo.links = off; off += align_up(4 * (size_t)(storage / 2) * V * 2 * w);
+    lo.delta = off; off += align_up(4 * V * 2 * w);
+    const size_t stage_sites = V < (size_t)kStageSites ? V : (size_t)kStageSites;
+    lo.staging = off; off += align_up(stage_sites * 36 * 2 * w);
+    lo.total = off;
+    return lo;
+}
+
+}  // namespace
+
+struct lgf_ctx {
+    int32_t L[4];
+    int precision, storage;
+    long long V;
+    size_t wbytes;               // bytes per real
+    char* ws;                    // device workspace
+    bool owns_ws;
+    cudaStream_t stream;
+    cudaStream_t cap_stream;     // library-owned stream used only to CAPTURE graphs (the legacy default stream cannot be captured)
+    Layout lo;
+    Geom geom;
+    Axis axis[4];
+    XyPass xy;                   // K2, K4
+    ZtPass zt;                   // K3
+    int xy_threads, zt_threads;
+    size_t xy_smem, zt_smem;
+    bool loaded, delta_valid;
+    int64_t launches;
+    // iteration graph (K2 K3 K4 K5 K1), captured per alpha
+    cudaGraphExec_t graph;
+    double graph_alpha;
+    int launches_per_iter;
+    // pinned host mirror of DevState (two slots for the lgf_fix polling pipeline)
+    DevState* host_state;
+    cudaEvent_t ev[2];
+    int64_t pending_n;           // lgf_iterate_async bookkeeping (-1: nothing pending)
+};
+
+namespace {
+
+DevState* dev_state(lgf_ctx* c) { return reinterpret_cast<DevState*>(c->ws + c->lo.state); }
+
+__global__ void init_state_kernel(DevState* st, double tol, long long max_iter) {
+    st->iter = 0;
+    st->done = 0;
+    st->ticket = 0;
+    st->tol = tol;
+    st->max_iter = max_iter;
+}
+// after the initial measurement of lgf_fix: already converged (or max_iter == 0)?
+__global__ void initial_test_kernel(DevState* st) {
+    if (st->theta < st->tol || st->max_iter <= 0) st->done = 1;
+}
+
+// ---- FFT pass planning -------------------------------------------------------------------------
+int threads_for(long long elems, const Axis& a, const Axis& b) {
+    long long need = 32;
+    const Axis* axes[2] = {&a, &b};
+    for (int i = 0; i < 2; ++i)
+        for (int s = 0; s < axes[i]->nstages; ++s) {
+            const int R = int((axes[i]->radices >> (4 * s)) & 15ull);
+            const int per_thread = R * (kElemsPerThread / R);
+            const long long t = (elems + per_thread - 1) / per_thread;
+            if (t > need) need = t;
+        }
+    need = (need + 31) / 32 * 32;
+    return need > 4096 ? 4096 : (int)need;
+}
+
+// returns false if a transform tile cannot be held on chip
+bool plan_passes(lgf_ctx* c) {
+    const int* L = c->L;
+    const size_t cb = 2 * c->wbytes;   // bytes per complex
+    const int max_threads = c->precision == LGF_F64 ? 512 : 1024;
+    for (int i = 0; i < 4; ++i) {
+        if (!factor23(L[i], &c->axis[i])) return false;
+        c->axis[i].tw_fwd = c->ws + c->lo.tw[i];
+        c->axis[i].tw_inv = c->ws + c->lo.twi[i];
+        c->axis[i].psq = c->ws + c->lo.psq[i];
+    }
+    const long long LxLy = (long long)L[0] * L[1], LzLt = (long long)L[2] * L[3];
+    // K2 / K4
+    c->xy.ax = c->axis[0];
+    c->xy.ay = c->axis[1];
+    c->xy.pitch = L[0] + 1;
+    c->xy_threads = threads_for(LxLy, c->axis[0], c->axis[1]);
+    c->xy_smem = (size_t)c->xy.pitch * L[1] * cb;
+    if (c->xy_threads > max_threads || c->xy_smem > (size_t)kMaxSmem) return false;
+    // K3: largest chunk of contiguous sites whose (z,t) plane fits (prefer <= 64 KB for occupancy)
+    int best = 0;
+    const size_t budgets[2] = {(size_t)64 * 1024, (size_t)kMaxSmem};
+    for (int pass = 0; pass < 2 && !best; ++pass)
+        for (int cx = 16; cx >= 1; cx /= 2) {
+            if (LxLy % cx) continue;
+            const size_t bytes = (size_t)cx * (L[2] + 1) * L[3] * cb;
+            if (bytes <= budgets[pass] && threads_for(cx * LzLt, c->axis[2], c->axis[3]) <= max_threads) { best = cx; break; }
+        }
+    if (!best) return false;
+    ZtPass& Z = c->zt;
+    Z.az = c->axis[2];
+    Z.at = c->axis[3];
+    Z.cx = best;
+    Z.pz = best;
+    Z.pt = best * (L[2] + 1);
+    Z.gz = LxLy;
+    Z.gt = LxLy * L[2];
+    Z.tiles_per_comp = (int)(LxLy / best);
+    Z.Lx = L[0];
+    Z.psq_x = c->axis[0].psq;
+    Z.psq_y = c->axis[1].psq;
+    double pmax = 0;
+    for (int i = 0; i < 4; ++i) {
+        const long double s = sinl(3.141592653589793238462643383279502884L * (long double)(L[i] / 2) / (long double)L[i]);
+        pmax += (double)(4.0L * s * s);
+    }
+    Z.scale_num = pmax / (double)c->V;
+    c->zt_threads = threads_for(best * LzLt, c->axis[2], c->axis[3]);
+    c->zt_smem = (size_t)Z.pt * L[3] * cb;
+    return true;
+}
+
+template <typename T>
+int upload_tables(lgf_ctx* c) {
+    for (int mu = 0; mu < 4; ++mu) {
+        const int n = c->L[mu];
+        std::vector<Cx<T>> tw(n), twi(n);
+        std::vector<T> psq(n);
+        for (int j = 0; j < n; ++j) {
+            // exact octant reduction is not needed at these sizes: long double keeps ~1e-19
+            const long double ang = 2.0L * 3.141592653589793238462643383279502884L * (long double)j / (long double)n;
+            tw[j] = Cx<T>((T)cosl(ang), (T)(-sinl(ang)));
+            twi[j] = Cx<T>((T)cosl(ang), (T)(sinl(ang)));
+            const long double s = sinl(3.141592653589793238462643383279502884L * (long double)j / (long double)n);
+            psq[j] = (T)(4.0L * s * s);
+        }
+        CU(cudaMemcpyAsync(c->ws + c->lo.tw[mu], tw.data(), n * sizeof(Cx<T>), cudaMemcpyHostToDevice, c->stream));
+        CU(cudaMemcpyAsync(c->ws + c->lo.twi[mu], twi.data(), n * sizeof(Cx<T>), cudaMemcpyHostToDevice, c->stream));
+        CU(cudaMemcpyAsync(c->ws + c->lo.psq[mu], psq.data(), n * sizeof(T), cudaMemcpyHostToDevice, c->stream));
+        CU(cudaStreamSynchronize(c->stream));   // the host vectors die at the end of this scope
+    }
+    return LGF_OK;
+}
+
+// ---- typed launchers ---------------------------------------------------------------------------
+template <typename T, int NC>
+struct Impl {
+    static Cx<T>* links(lgf_ctx* c) { return reinterpret_cast<Cx<T>*>(c->ws + c->lo.links); }
+    static Cx<T>* delta(lgf_ctx* c) { return reinterpret_cast<Cx<T>*>(c->ws + c->lo.delta); }
+    static Cx<T>* staging(lgf_ctx* c) { return reinterpret_cast<Cx<T>*>(c->ws + c->lo.staging); }
+
+    static int k1(lgf_ctx* c, int mode) {
+        k1_delta_theta_F<T, NC, TileA><<<c->lo.nblocks_site, TileA::kThreads, 0, c->stream>>>(
+            links(c), delta(c), reinterpret_cast<double2*>(c->ws + c->lo.partials), dev_state(c), c->geom, mode);
+        c->launches++;
+        CU(cudaGetLastError());
+        return LGF_OK;
+    }
+    static int k5(lgf_ctx* c, double alpha) {
+        k5_gbuild_update<T, NC, TileA><<<c->lo.nblocks_site, TileA::kThreads, 0, c->stream>>>(
+            links(c), delta(c), dev_state(c), c->geom, (T)(0.5 * alpha));
+        c->launches++;
+        CU(cudaGetLastError());
+        return LGF_OK;
+    }
+    static int fft(lgf_ctx* c, int k, bool gated) {
+        const int* done = gated ? &dev_state(c)->done : nullptr;
+        const unsigned planes = (unsigned)(4 * (long long)c->L[2] * c->L[3]);
+        if (k == 0)
+            fft_xy_kernel<T, -1><<<planes, c->xy_threads, c->xy_smem, c->stream>>>(delta(c), c->xy, done);
+        else if (k == 2)
+            fft_xy_kernel<T, +1><<<planes, c->xy_threads, c->xy_smem, c->stream>>>(delta(c), c->xy, done);
+        else
+            fft_zt_kernel<T><<<4 * c->zt.tiles_per_comp, c->zt_threads, c->zt_smem, c->stream>>>(delta(c), c->zt, c->V, done);
+        c->launches++;
+        CU(cudaGetLastError());
+        return LGF_OK;
+    }
+    static int setup(lgf_ctx* c) {
+        CU(cudaFuncSetAttribute(fft_xy_kernel<T, -1>, cudaFuncAttributeMaxDynamicSharedMemorySize, kMaxSmem));
+        CU(cudaFuncSetAttribute(fft_xy_kernel<T, +1>, cudaFuncAttributeMaxDynamicSharedMemorySize, kMaxSmem));
+        CU(cudaFuncSetAttribute(fft_zt_kernel<T>, cudaFuncAttributeMaxDynamicSharedMemorySize, kMaxSmem));
+        return upload_tables<T>(c);
+    }
+    static int load(lgf_ctx* c, const void* src, int memspace) {
+        const long long V = c->V;
+        const int thr = 256;
+        if (memspace == LGF_DEVICE) {
+            const long long n = V * 36;
+            aos_to_soa<T, NC><<<(unsigned)((n + thr - 1) / thr), thr, 0, c->stream>>>(
+                reinterpret_cast<const Cx<T>*>(src), links(c), V, 0, V);
+            c->launches++;
+            CU(cudaGetLastError());
+        } else {
+            const char* h = reinterpret_cast<const char*>(src);
+            for (long long s0 = 0; s0 < V; s0 += kStageSites) {
+                const long long ns = (V - s0 < kStageSites) ? V - s0 : kStageSites;
+                CU(cudaMemcpyAsync(staging(c), h + (size_t)s0 * 36 * sizeof(Cx<T>), (size_t)ns * 36 * sizeof(Cx<T>),
+                                   cudaMemcpyHostToDevice, c->stream));
+                const long long n = ns * 36;
+                aos_to_soa<T, NC><<<(unsigned)((n + thr - 1) / thr), thr, 0, c->stream>>>(staging(c), links(c), V, s0, ns);
+                c->launches++;
+                CU(cudaGetLastError());
+            }
+        }
+        CU(cudaStreamSynchronize(c->stream));
+        return LGF_OK;
+    }
+    static int store(lgf_ctx* c, void* dst, int memspace) {
+        const long long V = c->V;
+        const int thr = 256;
+        if (memspace == LGF_DEVICE) {
+            const long long n = V * 4;
+            soa_to_aos<T, NC><<<(unsigned)((n + thr - 1) / thr), thr, 0, c->stream>>>(
+                links(c), reinterpret_cast<Cx<T>*>(dst), V, 0, V);
+            c->launches++;
+            CU(cudaGetLastError());
+        } else {
+            char* h = reinterpret_cast<char*>(dst);
+            for (long long s0 = 0; s0 < V; s0 += kStageSites) {
+                const long long ns = (V - s0 < kStageSites) ? V - s0 : kStageSites;
+                const long long n = ns * 4;
+                soa_to_aos<T, NC><<<(unsigned)((n + thr - 1) / thr), thr, 0, c->stream>>>(links(c), staging(c), V, s0, ns);
+                c->launches++;
+                CU(cudaGetLastError());
+                CU(cudaMemcpyAsync(h + (size_t)s0 * 36 * sizeof(Cx<T>), staging(c), (size_t)ns * 36 * sizeof(Cx<T>),
+                                   cudaMemcpyDeviceToHost, c->stream));
+            }
+        }
+        CU(cudaStreamSynchronize(c->stream));
+        return LGF_OK;
+    }
+    static int get_delta(lgf_ctx* c, void* dst, int memspace) {
+        const long long V = c->V;
+        const int thr = 256;
+        if (memspace == LGF_DEVICE) {
+            delta_to_aos<T><<<(unsigned)((V * 4 + thr - 1) / thr), thr, 0, c->stream>>>(delta(c), reinterpret_cast<Cx<T>*>(dst), V);
+            c->launches++;
+            CU(cudaGetLastError());
+            CU(cudaStreamSynchronize(c->stream));
+            return LGF_OK;
+        }
+        // host: copy the four component planes and interleave on the host side of the copy
+        std::vector<Cx<T>> tmp((size_t)4 * V);
+        CU(cudaMemcpyAsync(tmp.data(), delta(c), (size_t)4 * V * sizeof(Cx<T>), cudaMemcpyDeviceToHost, c->stream));
+        CU(cudaStreamSynchronize(c->stream));
+        Cx<T>* out = reinterpret_cast<Cx<T>*>(dst);
+        for (long long s = 0; s < V; ++s)
+            for (int k = 0; k < 4; ++k) out[s * 4 + k] = tmp[(size_t)k * V + s];
+        return LGF_OK;
+    }
+};
+
+#define DISPATCH(c, CALL)                                                     \
+    ((c)->precision == LGF_F64                                                \
+         ? ((c)->storage == LGF_REAL18 ? Impl<double, 9>::CALL : Impl<double, 6>::CALL) \
+         : ((c)->storage == LGF_REAL18 ? Impl<float, 9>::CALL : Impl<float, 6>::CALL))
+
+int enqueue_iteration_body(lgf_ctx* c, double alpha) {
+    int rc;
+    if ((rc = DISPATCH(c, fft(c, 0, true)))) return rc;
+    if ((rc = DISPATCH(c, fft(c, 1, true)))) return rc;
+    if ((rc = DISPATCH(c, fft(c, 2, true)))) return rc;
+    if ((rc = DISPATCH(c, k5(c, alpha)))) return rc;
+    if ((rc = DISPATCH(c, k1(c, 1)))) return rc;
+    return LGF_OK;
+}
+
+// (Re)capture the iteration body into a CUDA graph for this alpha.
+int ensure_graph(lgf_ctx* c, double alpha) {
+    if (c->graph && c->graph_alpha == alpha) return LGF_OK;
+    if (c->graph) { cudaGraphExecDestroy(c->graph); c->graph = nullptr; }
+    const int64_t before = c->launches;
+    CU(cudaStreamBeginCapture(c->cap_stream, cudaStreamCaptureModeThreadLocal));
+    cudaStream_t user = c->stream;
+    c->stream = c->cap_stream;
+    const int rc = enqueue_iteration_body(c, alpha);
+    c->stream = user;
+    cudaGraph_t g = nullptr;
+    cudaError_t e = cudaStreamEndCapture(c->cap_stream, &g);
+    c->launches_per_iter = (int)(c->launches - before);
+    c->launches = before;   // capture launches nothing
+    if (rc) { if (g) cudaGraphDestroy(g); return rc; }
+    if (e != cudaSuccess) return cuda_fail(e, "cudaStreamEndCapture");
+    e = cudaGraphInstantiate(&c->graph, g, 0);
+    cudaGraphDestroy(g);
+    if (e != cudaSuccess) { c->graph = nullptr; return cuda_fail(e, "cudaGraphInstantiate"); }
+    c->graph_alpha = alpha;
+    return LGF_OK;
+}
+
+int enqueue_iterations(lgf_ctx* c, int64_t n) {
+    for (int64_t i = 0; i < n; ++i) {
+        CU(cudaGraphLaunch(c->graph, c->stream));
+        c->launches += c->launches_per_iter;
+    }
+    return LGF_OK;
+}
+
+int init_state(lgf_ctx* c, double tol, long long max_iter) {
+    init_state_kernel<<<1, 1, 0, c->stream>>>(dev_state(c), tol, max_iter);
+    c->launches++;
+    CU(cudaGetLastError());
+    return LGF_OK;
+}
+
+int fetch_state(lgf_ctx* c, int slot) {
+    CU(cudaMemcpyAsync(&c->host_state[slot], dev_state(c), sizeof(DevState), cudaMemcpyDeviceToHost, c->stream));
+    return LGF_OK;
+}
+
+}  // namespace
+
+// =================================================================================================
+extern "C" {
+
+const char* lgf_version(void) { return "0.1"; }
+const char* lgf_last_error(void) { return g_last_error; }
+
+const char* lgf_strerror(int code) {
+    switch (code) {
+        case LGF_OK: return "ok";
+        case LGF_EINVAL: return "invalid argument";
+        case LGF_EUNSUPPORTED: return "unsupported lattice (extent not 2^a 3^b, or transform tile exceeds shared memory)";
+        case LGF_ESTATE: return "no links loaded";
+        case LGF_ECUDA: return "CUDA error (see lgf_last_error)";
+        default: return "unknown error";
+    }
+}
+
+size_t lgf_workspace_bytes(const int32_t L[4], int precision, int storage) {
+    if (!valid_args(L, precision, storage)) return 0;
+    Axis ax;
+    for (int i = 0; i < 4; ++i)
+        if (!factor23(L[i], &ax)) return 0;
+    return make_layout(L, precision, storage).total;
+}
+
+static int create_common(const int32_t L[4], int precision, int storage, void* ws, size_t ws_bytes, bool owns,
+                         void* stream, lgf_ctx** out) {
+    lgf_ctx* c = new (std::nothrow) lgf_ctx();
+    if (!c) return LGF_EINVAL;
+    memset(c, 0, sizeof(*c));
+    for (int i = 0; i < 4; ++i) c->L[i] = L[i];
+    c->precision = precision;
+    c->storage = storage;
+    c->V = (long long)L[0] * L[1] * L[2] * L[3];
+    c->wbytes = precision == LGF_F64 ? 8 : 4;
+    c->ws = reinterpret_cast<char*>(ws);
+    c->owns_ws = owns;
+    c->stream = reinterpret_cast<cudaStream_t>(stream);
+    c->lo = make_layout(L, precision, storage);
+    c->pending_n = -1;
+    for (int i = 0; i < 4; ++i) { c->geom.L[i] = L[i]; c->geom.nb[i] = c->lo.nb[i]; }
+    c->geom.V = c->V;
+    int rc = LGF_OK;
+    if (ws_bytes < c->lo.total || (reinterpret_cast<uintptr_t>(ws) % kAlign) != 0) rc = LGF_EINVAL;
+    if (!rc && !plan_passes(c)) rc = LGF_EUNSUPPORTED;
+    if (!rc) {
+        cudaError_t e = cudaMallocHost(reinterpret_cast<void**>(&c->host_state), 2 * sizeof(DevState));
+        if (e != cudaSuccess) rc = cuda_fail(e, "cudaMallocHost");
+    }
+    if (!rc) {
+        cudaError_t e = cudaStreamCreateWithFlags(&c->cap_stream, cudaStreamNonBlocking);
+        if (e != cudaSuccess) rc = cuda_fail(e, "cudaStreamCreateWithFlags");
+    }
+    for (int i = 0; i < 2 && !rc; ++i) {
+        cudaError_t e = cudaEventCreateWithFlags(&c->ev[i], cudaEventDisableTiming);
+        if (e != cudaSuccess) rc = cuda_fail(e, "cudaEventCreate");
+    }
+    if (!rc) rc = DISPATCH(c, setup(c));
+    if (!rc) rc = init_state(c, -1.0, 0);
+    if (!rc) {
+        cudaError_t e = cudaStreamSynchronize(c->stream);
+        if (e != cudaSuccess) rc = cuda_fail(e, "cudaStreamSynchronize");
+    }
+    if (rc) {
+        c->owns_ws = false;   // the caller of create_common frees on failure
+        lgf_destroy(c);
+        return rc;
+    }
+    *out = c;
+    return LGF_OK;
+}
+
+int lgf_create(const int32_t L[4], int precision, int storage, void* workspace_dev, size_t workspace_bytes,
+               void* cuda_stream, lgf_ctx** out) {
+    if (!out || !workspace_dev || !valid_args(L, precision, storage)) return LGF_EINVAL;
+    if (lgf_workspace_bytes(L, precision, storage) == 0) return LGF_EUNSUPPORTED;
+    return create_common(L, precision, storage, workspace_dev, workspace_bytes, false, cuda_stream, out);
+}
+
+int lgf_create_simple(const int32_t L[4], int precision, int storage, lgf_ctx** out) {
+    if (!out || !valid_args(L, precision, storage)) return LGF_EINVAL;
+    const size_t bytes = lgf_workspace_bytes(L, precision, storage);
+    if (bytes == 0) return LGF_EUNSUPPORTED;
+    void* ws = nullptr;
+    CU(cudaMalloc(&ws, bytes));
+    const int rc = create_common(L, precision, storage, ws, bytes, true, nullptr, out);
+    if (rc) cudaFree(ws);
+    return rc;
+}
+
+int lgf_destroy(lgf_ctx* c) {
+    if (!c) return LGF_EINVAL;
+    if (c->stream || c->ws) cudaStreamSynchronize(c->stream);
+    if (c->graph) cudaGraphExecDestroy(c->graph);
+    if (c->cap_stream) cudaStreamDestroy(c->cap_stream);
+    for (int i = 0; i < 2; ++i)
+        if (c->ev[i]) cudaEventDestroy(c->ev[i]);
+    if (c->host_state) cudaFreeHost(c->host_state);
+    if (c->owns_ws && c->ws) cudaFree(c->ws);
+    delete c;
+    return LGF_OK;
+}
+
+int lgf_load(lgf_ctx* c, const void* links, int memspace) {
+    if (!c || !links || (memspace != LGF_HOST && memspace != LGF_DEVICE)) return LGF_EINVAL;
+    const int rc = DISPATCH(c, load(c, links, memspace));
+    if (rc) return rc;
+    c->loaded = true;
+    c->delta_valid = false;
+    return LGF_OK;
+}
+
+int lgf_store(lgf_ctx* c, void* links, int memspace) {
+    if (!c || !links || (memspace != LGF_HOST && memspace != LGF_DEVICE)) return LGF_EINVAL;
+    if (!c->loaded) return LGF_ESTATE;
+    return DISPATCH(c, store(c, links, memspace));
+}
+
+static int finish(lgf_ctx* c, lgf_result* out, bool fix_mode) {
+    int rc = fetch_state(c, 0);
+    if (rc) return rc;
+    CU(cudaStreamSynchronize(c->stream));
+    const DevState& s = c->host_state[0];
+    if (out) {
+        out->iterations = s.iter;
+        out->theta = s.theta;
+        out->F = s.F;
+        out->converged = fix_mode ? (s.theta < s.tol ? 1 : 0) : 0;
+    }
+    return LGF_OK;
+}
+
+int lgf_measure(lgf_ctx* c, lgf_result* out) {
+    if (!c || !out) return LGF_EINVAL;
+    if (!c->loaded) return LGF_ESTATE;
+    int rc = init_state(c, -1.0, 0);
+    if (!rc) rc = DISPATCH(c, k1(c, 0));
+    if (rc) return rc;
+    c->delta_valid = true;
+    lgf_result r;
+    rc = finish(c, &r, false);
+    if (rc) return rc;
+    r.iterations = 0;
+    *out = r;
+    return LGF_OK;
+}
+
+int lgf_iterate_async(lgf_ctx* c, int64_t n, double alpha) {
+    if (!c || n < 0 || !(alpha > 0)) return LGF_EINVAL;
+    if (!c->loaded) return LGF_ESTATE;
+    int rc = ensure_graph(c, alpha);
+    if (!rc) rc = init_state(c, -1.0, (long long)n);
+    if (!rc && (!c->delta_valid || n == 0)) rc = DISPATCH(c, k1(c, 0));
+    if (!rc) { c->delta_valid = true; rc = enqueue_iterations(c, n); }
+    if (rc) return rc;
+    c->pending_n = n;
+    return LGF_OK;
+}
+
+int lgf_wait(lgf_ctx* c, lgf_result* out) {
+    if (!c) return LGF_EINVAL;
+    if (c->pending_n < 0) return LGF_ESTATE;
+    lgf_result r;
+    const int rc = finish(c, &r, false);
+    c->pending_n = -1;
+    if (rc) return rc;
+    if (out) *out = r;
+    return LGF_OK;
+}
+
+int lgf_iterate(lgf_ctx* c, int64_t n, double alpha, lgf_result* out) {
+    if (!out) return LGF_EINVAL;
+    const int rc = lgf_iterate_async(c, n, alpha);
+    if (rc) return rc;
+    return lgf_wait(c, out);
+}
+
+int lgf_fix(lgf_ctx* c, double alpha, double theta_tol, int64_t max_iter, lgf_result* out) {
+    if (!c || !out || !(alpha > 0) || max_iter < 0 || !(theta_tol == theta_tol)) return LGF_EINVAL;
+    if (!c->loaded) return LGF_ESTATE;
+    int rc = ensure_graph(c, alpha);
+    if (!rc) rc = init_state(c, theta_tol, (long long)max_iter);
+    if (!rc) rc = DISPATCH(c, k1(c, 0));
+    if (rc) return rc;
+    c->delta_valid = true;
+    initial_test_kernel<<<1, 1, 0, c->stream>>>(dev_state(c));
+    c->launches++;
+    CU(cudaGetLastError());
+    // Batches of kFixBatch gated iterations; the state block is copied to pinned memory after each
+    // batch.  The host keeps one batch in flight ahead of the one it polls, so the GPU never idles
+    // waiting for the host; iterations enqueued past the crossing are no-ops (DevState::done).
+    int64_t enq = 0;
+    int slot = 0;
+    bool have_prev = false;
+    int prev_slot = 0;
+    bool done = false;
+    while (!done) {
+        const int64_t nb = (max_iter - enq < kFixBatch) ? max_iter - enq : kFixBatch;
+        if (nb > 0) {
+            if ((rc = enqueue_iterations(c, nb))) return rc;
+            enq += nb;
+        }
+        if ((rc = fetch_state(c, slot))) return rc;
+        CU(cudaEventRecord(c->ev[slot], c->stream));
+        if (have_prev) {
+            CU(cudaEventSynchronize(c->ev[prev_slot]));
+            if (c->host_state[prev_slot].done) done = true;
+        }
+        if (nb <= 0 || enq >= max_iter) {
+            // nothing more to enqueue: drain the last batch
+            CU(cudaEventSynchronize(c->ev[slot]));
+            done = true;
+        }
+        have_prev = true;
+        prev_slot = slot;
+        slot ^= 1;
+    }
+    return finish(c, out, true);
+}
+
+int lgf_debug_get_delta(lgf_ctx* c, void* delta_packed, int memspace) {
+    if (!c || !delta_packed || (memspace != LGF_HOST && memspace != LGF_DEVICE)) return LGF_EINVAL;
+    if (!c->loaded) return LGF_ESTATE;
+    return DISPATCH(c, get_delta(c, delta_packed, memspace));
+}
+
+int lgf_debug_fourier_accelerate(lgf_ctx* c) {
+    if (!c) return LGF_EINVAL;
+    if (!c->loaded || !c->delta_valid) return LGF_ESTATE;
+    int rc;
+    for (int k = 0; k < 3; ++k)
+        if ((rc = DISPATCH(c, fft(c, k, false)))) return rc;
+    c->delta_valid = false;
+    CU(cudaStreamSynchronize(c->stream));
+    return LGF_OK;
+}
+
+int lgf_profile_iterate(lgf_ctx* c, int64_t n, double alpha, double ms[5], lgf_result* out) {
+    if (!c || !ms || n <= 0 || !(alpha > 0)) return LGF_EINVAL;
+    if (!c->loaded) return LGF_ESTATE;
+    int rc = init_state(c, -1.0, (long long)n);
+    if (!rc && !c->delta_valid) rc = DISPATCH(c, k1(c, 0));
+    if (rc) return rc;
+    c->delta_valid = true;
+    cudaEvent_t ev[6];
+    for (int i = 0; i < 6; ++i) CU(cudaEventCreate(&ev[i]));
+    double acc[5] = {0, 0, 0, 0, 0};
+    for (int64_t it = 0; it < n && !rc; ++it) {
+        for (int k = 0; k < 5 && !rc; ++k) {
+            CU(cudaEventRecord(ev[k], c->stream));
+            if (k < 3) rc = DISPATCH(c, fft(c, k, true));
+            else if (k == 3) rc = DISPATCH(c, k5(c, alpha));
+            else rc = DISPATCH(c, k1(c, 1));
+        }
+        if (rc) break;
+        CU(cudaEventRecord(ev[5], c->stream));
+        CU(cudaEventSynchronize(ev[5]));
+        for (int k = 0; k < 5; ++k) {
+            float t = 0;
+            CU(cudaEventElapsedTime(&t, ev[k], ev[k + 1]));
+            acc[k] += t;
+        }
+    }
+    for (int i = 0; i < 6; ++i) cudaEventDestroy(ev[i]);
+    if (rc) return rc;
+    for (int k = 0; k < 5; ++k) ms[k] = acc[k] / (double)n;
+    lgf_result r;
+    rc = finish(c, &r, false);
+    if (rc) return rc;
+    if (out) *out = r;
+    return LGF_OK;
+}
+
+int64_t lgf_launch_count(const lgf_ctx* c) { return c ? c->launches : 0; }
+
+}  // extern "C"

@@ -1,0 +1,258 @@
+// lgf_site.cuh -- per-site kernels: K1 (Delta / theta / F), K5 (g-build + link update),
+// boundary layout transposes.  Product code (sm_100a); shares nothing with oracle/.
+//
+// Device layouts:
+//   links  U[mu][c][s]  complex<T>, c = 0..NC-1 row-major matrix element (NC = 9: 18-real,
+//                       NC = 6: rows 0,1 only = 12-real), s lexicographic x fastest
+//   Delta  D[c][s]      complex<T>, c = 0..3 packed: D01, D02, D12, Im D00 + i Im D11
+#pragma once
+#include "lgf_math.cuh"
+
+namespace lgf {
+
+struct Geom {
+    int L[4];    // Lx, Ly, Lz, Lt
+    int nb[4];   // tiles per axis for the per-site kernels
+    long long V;
+};
+
+// Loop / reduction state, lives in the workspace (device memory).
+struct DevState {
+    double theta;
+    double F;
+    long long iter;          // link updates applied since the run started
+    int done;                // 1: theta < tol reached (or max_iter) -> later kernels are no-ops
+    unsigned int ticket;     // K1 block counter for the last-block reduction
+    double tol;
+    long long max_iter;
+};
+
+template <int TX, int TY, int TZ, int TT>
+struct SiteTile {
+    static constexpr int kThreads = TX * TY * TZ * TT;
+    // thread -> lattice coordinates of its site; returns false outside the lattice
+    __device__ static __forceinline__ bool coords(const Geom& g, int x[4]) {
+        int b = blockIdx.x;
+        const int bx = b % g.nb[0]; b /= g.nb[0];
+        const int by = b % g.nb[1]; b /= g.nb[1];
+        const int bz = b % g.nb[2]; b /= g.nb[2];
+        const int bt = b;
+        int t = threadIdx.x;
+        x[0] = bx * TX + t % TX; t /= TX;
+        x[1] = by * TY + t % TY; t /= TY;
+        x[2] = bz * TZ + t % TZ; t /= TZ;
+        x[3] = bt * TT + t;
+        return x[0] < g.L[0] && x[1] < g.L[1] && x[2] < g.L[2] && x[3] < g.L[3];
+    }
+};
+
+__device__ __forceinline__ long long site_index(const Geom& g, const int x[4]) {
+    return x[0] + (long long)g.L[0] * (x[1] + (long long)g.L[1] * (x[2] + (long long)g.L[2] * x[3]));
+}
+__device__ __forceinline__ long long axis_stride(const Geom& g, int mu) {
+    long long s = 1;
+    for (int i = 0; i < mu; ++i) s *= g.L[i];
+    return s;
+}
+
+// Load one link into registers; in 12-real mode rebuild row 2.
+template <typename T, int NC>
+__device__ __forceinline__ void load_link(Su3<T>& u, const Cx<T>* __restrict__ U, long long V, int mu, long long s) {
+    const Cx<T>* p = U + (size_t)mu * NC * V + s;
+#pragma unroll
+    for (int c = 0; c < NC; ++c) u.m[c] = ld_cx(p + (size_t)c * V);
+    if (NC == 6) rebuild_row2(u);
+}
+
+// Deterministic block reduction of two doubles; result valid in thread 0.
+template <int NT>
+__device__ __forceinline__ void block_sum2(double& a, double& b) {
+    __shared__ double sa[NT / 32], sb[NT / 32];
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) {
+        a += __shfl_down_sync(0xffffffffu, a, o);
+        b += __shfl_down_sync(0xffffffffu, b, o);
+    }
+    const int w = threadIdx.x >> 5, l = threadIdx.x & 31;
+    if (l == 0) { sa[w] = a; sb[w] = b; }
+    __syncthreads();
+    if (w == 0) {
+        a = (l < NT / 32) ? sa[l] : 0.0;
+        b = (l < NT / 32) ? sb[l] : 0.0;
+#pragma unroll
+        for (int o = 16; o > 0; o >>= 1) {
+            a += __shfl_down_sync(0xffffffffu, a, o);
+            b += __shfl_down_sync(0xffffffffu, b, o);
+        }
+    }
+}
+
+// ---------------------------------------------------------------------------------------------
+// K1  delta_theta_F  (north_star step 1)
+//   M(x) = sum_mu [U_mu(x-mu) - U_mu(x)],  A = M - M^+,  Delta = A - (Tr A/3) 1  -> packed 4 complex
+//   theta = (1/(3V)) sum |Delta_ij|^2,  F = (1/(12V)) sum Re Tr U_mu(x); sums in fp64, fixed order.
+// mode: 0 = plain measurement; 1 = end of an iteration (skipped if st->done, bumps st->iter and
+// evaluates the stopping test theta < tol / iter >= max_iter on the device).
+// ---------------------------------------------------------------------------------------------
+template <typename T, int NC, class Tile>
+__global__ void __launch_bounds__(Tile::kThreads)
+k1_delta_theta_F(const Cx<T>* __restrict__ U, Cx<T>* __restrict__ D, double2* __restrict__ partials,
+                 DevState* st, Geom g, int mode) {
+    if (mode == 1 && *reinterpret_cast<volatile int*>(&st->done)) return;
+    int x[4];
+    const bool valid = Tile::coords(g, x);
+    double th = 0.0, fn = 0.0;
+    if (valid) {
+        const long long s = site_index(g, x);
+        Su3<T> M;
+#pragma unroll
+        for (int c = 0; c < 9; ++c) M.m[c] = Cx<T>(0, 0);
+        T retr = 0;
+        long long stride = 1;
+#pragma unroll
+        for (int mu = 0; mu < 4; ++mu) {
+            const long long sb = (x[mu] == 0) ? s + stride * (g.L[mu] - 1) : s - stride;
+            Su3<T> a, b;
+            load_link<T, NC>(a, U, g.V, mu, s);
+            load_link<T, NC>(b, U, g.V, mu, sb);
+#pragma unroll
+            for (int c = 0; c < 9; ++c) M.m[c] = M.m[c] + (b.m[c] - a.m[c]);
+            retr += a.m[0].re + a.m[4].re + a.m[8].re;
+            stride *= g.L[mu];
+        }
+        // A = M - M^+ : off-diagonals A01, A02, A12; diagonal i * 2 Im M_ii; remove trace/3
+        const Cx<T> c0 = M.m[1] - conj(M.m[3]);
+        const Cx<T> c1 = M.m[2] - conj(M.m[6]);
+        const Cx<T> c2 = M.m[5] - conj(M.m[7]);
+        const T a0 = T(2) * M.m[0].im, a1 = T(2) * M.m[4].im, a2 = T(2) * M.m[8].im;
+        const T tr3 = (a0 + a1 + a2) / T(3);
+        const T d0 = a0 - tr3, d1 = a1 - tr3, d2 = a2 - tr3;
+        st_cx(D + s, c0);
+        st_cx(D + (size_t)g.V + s, c1);
+        st_cx(D + (size_t)2 * g.V + s, c2);
+        st_cx(D + (size_t)3 * g.V + s, Cx<T>(d0, d1));
+        th = 2.0 * ((double)norm2(c0) + (double)norm2(c1) + (double)norm2(c2)) + (double)d0 * d0 +
+             (double)d1 * d1 + (double)d2 * d2;
+        fn = (double)retr;
+    }
+    block_sum2<Tile::kThreads>(th, fn);
+    __shared__ bool is_last;
+    if (threadIdx.x == 0) {
+        partials[blockIdx.x] = make_double2(th, fn);
+        __threadfence();
+        const unsigned int t = atomicAdd(&st->ticket, 1u);
+        is_last = (t == gridDim.x - 1);
+    }
+    __syncthreads();
+    if (!is_last) return;
+    __threadfence();
+    // last block: fixed-order sum of all partials (independent of which block came last)
+    double a = 0.0, b = 0.0;
+    for (unsigned int i = threadIdx.x; i < gridDim.x; i += Tile::kThreads) {
+        const double2 p = __ldcg(partials + i);
+        a += p.x;
+        b += p.y;
+    }
+    block_sum2<Tile::kThreads>(a, b);
+    if (threadIdx.x == 0) {
+        const double theta = a / (3.0 * (double)g.V);
+        st->theta = theta;
+        st->F = b / (12.0 * (double)g.V);
+        st->ticket = 0;
+        if (mode == 1) {
+            const long long it = st->iter + 1;
+            st->iter = it;
+            if (theta < st->tol || it >= st->max_iter) st->done = 1;
+        }
+        __threadfence();
+    }
+}
+
+// ---------------------------------------------------------------------------------------------
+// K5  gbuild_update  (north_star steps 4, 5)
+//   g(y) = reunitarise(1 + (alpha/2) Dt(y)) for y = x and the four forward neighbours,
+//   U'_mu(x) = g(x) U_mu(x) g(x+mu)^+, in place (each link is read and written by one thread only).
+// ---------------------------------------------------------------------------------------------
+template <typename T>
+__device__ __forceinline__ void load_g(Su3<T>& g, const Cx<T>* __restrict__ D, long long V, long long s, T ha) {
+    const Cx<T> c0 = ld_cx(D + s), c1 = ld_cx(D + (size_t)V + s), c2 = ld_cx(D + (size_t)2 * V + s),
+                c3 = ld_cx(D + (size_t)3 * V + s);
+    build_g(g, c0, c1, c2, c3, ha);
+}
+
+template <typename T, int NC, class Tile>
+__global__ void __launch_bounds__(Tile::kThreads)
+k5_gbuild_update(Cx<T>* __restrict__ U, const Cx<T>* __restrict__ D, const DevState* st, Geom g, T half_alpha) {
+    if (*reinterpret_cast<const volatile int*>(&st->done)) return;
+    int x[4];
+    if (!Tile::coords(g, x)) return;
+    const long long s = site_index(g, x);
+    constexpr int NR = NC / 3;  // rows to produce: 3 or 2
+    Su3<T> g0;
+    load_g(g0, D, g.V, s, half_alpha);
+    long long stride = 1;
+#pragma unroll
+    for (int mu = 0; mu < 4; ++mu) {
+        const long long sf = (x[mu] == g.L[mu] - 1) ? s - stride * (g.L[mu] - 1) : s + stride;
+        Su3<T> gf, u;
+        load_g(gf, D, g.V, sf, half_alpha);
+        load_link<T, NC>(u, U, g.V, mu, s);
+        // W = g0 * u (rows 0..NR-1), then U' = W * gf^+
+        Cx<T> W[3 * NR];
+#pragma unroll
+        for (int i = 0; i < NR; ++i)
+#pragma unroll
+            for (int j = 0; j < 3; ++j) {
+                Cx<T> acc = g0.m[3 * i] * u.m[j];
+                fma_cx(acc, g0.m[3 * i + 1], u.m[3 + j]);
+                fma_cx(acc, g0.m[3 * i + 2], u.m[6 + j]);
+                W[3 * i + j] = acc;
+            }
+        Cx<T>* p = U + (size_t)mu * NC * g.V + s;
+#pragma unroll
+        for (int i = 0; i < NR; ++i)
+#pragma unroll
+            for (int j = 0; j < 3; ++j) {
+                Cx<T> acc = mulc(W[3 * i], gf.m[3 * j]);
+                fma_cxc(acc, W[3 * i + 1], gf.m[3 * j + 1]);
+                fma_cxc(acc, W[3 * i + 2], gf.m[3 * j + 2]);
+                st_cx(p + (size_t)(3 * i + j) * g.V, acc);
+            }
+        stride *= g.L[mu];
+    }
+}
+
+// ---------------------------------------------------------------------------------------------
+// Boundary transposes: AoS links[s][mu][3][3] (complex<T>) <-> device U[mu][c][s].
+// `aos` points at site `s0`; n sites are converted.
+// ---------------------------------------------------------------------------------------------
+template <typename T, int NC>
+__global__ void aos_to_soa(const Cx<T>* __restrict__ aos, Cx<T>* __restrict__ U, long long V, long long s0, long long n) {
+    const long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x;  // over n * 36
+    if (i >= n * 36) return;
+    const long long sl = i / 36;
+    const int r = int(i - sl * 36), mu = r / 9, c = r % 9;
+    if (c < NC) U[(size_t)(mu * NC + c) * V + s0 + sl] = aos[i];
+}
+
+template <typename T, int NC>
+__global__ void soa_to_aos(const Cx<T>* __restrict__ U, Cx<T>* __restrict__ aos, long long V, long long s0, long long n) {
+    const long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x;  // over n * 4
+    if (i >= n * 4) return;
+    const long long sl = i / 4;
+    const int mu = int(i - sl * 4);
+    Su3<T> u;
+    load_link<T, NC>(u, U, V, mu, s0 + sl);
+#pragma unroll
+    for (int c = 0; c < 9; ++c) aos[i * 9 + c] = u.m[c];
+}
+
+// packed Delta D[c][s] -> [s][4] (debug/inspection hook)
+template <typename T>
+__global__ void delta_to_aos(const Cx<T>* __restrict__ D, Cx<T>* __restrict__ out, long long V) {
+    const long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= V * 4) return;
+    out[i] = D[(size_t)(i & 3) * V + (i >> 2)];
+}
+
+}  // namespace lgf

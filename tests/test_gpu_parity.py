@@ -1,0 +1,207 @@
+"""GPU parity: the CUDA path (through the C ABI) against the oracle on the same seeded inputs.
+Tolerances are north_star's: fp64 links after 1 iteration max|dU| <= 1e-12; theta, F at convergence
+relative 1e-10 and identical iteration counts; fp32 per-iteration links <= 2e-5, F relative 1e-5."""
+import numpy as np
+import pytest
+import torch
+
+import lgf_inputs as gi
+import oracle
+import paper_1208_1186_b200 as lgf
+
+pytestmark = pytest.mark.gpu
+ALPHA = 0.08
+
+SHAPES = [(8, 8, 8, 8), (6, 4, 12, 8), (4, 6, 3, 2), (16, 8, 4, 12), (12, 12, 6, 4), (2, 2, 2, 2), (24, 18, 4, 8)]
+MODES = [(lgf.LGF_F64, lgf.LGF_REAL18), (lgf.LGF_F64, lgf.LGF_REAL12)]
+
+
+def _pack(D):
+    """oracle Delta [V,3,3] -> packed [V,4] complex."""
+    return np.stack([D[:, 0, 1], D[:, 0, 2], D[:, 1, 2], D[:, 0, 0].imag + 1j * D[:, 1, 1].imag], 1)
+
+
+def _cplx(t):
+    return torch.view_as_complex(t.to(torch.float64).contiguous()).numpy()
+
+
+def _fixer(L, prec, stor, U):
+    dt = torch.float64 if prec == lgf.LGF_F64 else torch.float32
+    gf = lgf.GaugeFixer(L, prec, stor)
+    gf.load(gi.as_real(U, dt))
+    return gf
+
+
+@pytest.mark.parametrize("L", SHAPES)
+@pytest.mark.parametrize("prec,stor", MODES)
+def test_k1_delta_theta_F(L, prec, stor):
+    U = gi.make_config(L, 21, 0.59)
+    D, theta, F = oracle.measure(L, U)
+    gf = _fixer(L, prec, stor, U)
+    r = gf.measure()
+    got = _cplx(gf.debug_delta())
+    assert np.max(np.abs(got - _pack(D))) <= 2e-14
+    assert abs(r.theta - theta) <= 1e-13 * theta
+    assert abs(r.F - F) <= 1e-13 * max(abs(F), 1e-3)
+    assert r.iterations == 0
+    gf.close()
+
+
+@pytest.mark.parametrize("L", SHAPES)
+def test_k2_k3_k4_fourier_acceleration(L):
+    U = gi.make_config(L, 22, 0.59)
+    D, _, _ = oracle.measure(L, U)
+    Dt = _pack(oracle.fourier_accelerate(L, D))      # oracle transforms all 9 elements (pin P10)
+    gf = _fixer(L, lgf.LGF_F64, lgf.LGF_REAL18, U)
+    gf.measure()
+    gf.debug_fourier_accelerate()
+    got = _cplx(gf.debug_delta())
+    assert np.max(np.abs(got - Dt)) <= 1e-13 * max(1.0, np.max(np.abs(Dt)))
+    gf.close()
+
+
+@pytest.mark.parametrize("L", SHAPES)
+@pytest.mark.parametrize("prec,stor", MODES)
+def test_one_iteration_links_fp64(L, prec, stor):
+    U = gi.make_config(L, 23, 0.59)
+    ref, thh, Fh = oracle.iterate(L, U, 1, ALPHA)
+    gf = _fixer(L, prec, stor, U)
+    r = gf.iterate(1, ALPHA)
+    got = _cplx(gf.store())
+    assert np.max(np.abs(got - ref)) <= 1e-12
+    assert r.iterations == 1
+    assert abs(r.theta - thh[1]) <= 1e-11 * thh[1]
+    assert abs(r.F - Fh[1]) <= 1e-12
+    gf.close()
+
+
+@pytest.mark.parametrize("L", [(8, 8, 8, 8), (6, 4, 12, 8)])
+@pytest.mark.parametrize("prec,stor", MODES)
+def test_five_iterations_track_oracle(L, prec, stor):
+    U = gi.make_config(L, 24, 0.59)
+    ref, thh, Fh = oracle.iterate(L, U, 5, ALPHA)
+    gf = _fixer(L, prec, stor, U)
+    r = gf.iterate(5, ALPHA)
+    got = _cplx(gf.store())
+    assert np.max(np.abs(got - ref)) <= 1e-11
+    assert abs(r.theta - thh[5]) <= 1e-10 * thh[5]
+    # unitarity, det = 1 (P4)
+    g = torch.from_numpy(got)
+    eye = torch.eye(3, dtype=torch.complex128)
+    assert float((g @ g.conj().transpose(-1, -2) - eye).abs().max()) < 1e-13
+    assert float((torch.linalg.det(g) - 1).abs().max()) < 1e-13
+    # plaquette invariance (P5), via lgf_inputs' independent code
+    assert abs(gi.mean_plaquette(g, L) - gi.mean_plaquette(U, L)) < 1e-13
+    gf.close()
+
+
+def test_config0_convergence_8x4_fp64_18():
+    """configs[0]: 8^4 fp64 18-real, plaquette 0.59, alpha 0.08, theta < 1e-12 or 5000 iterations."""
+    L = (8, 8, 8, 8)
+    U = gi.make_config(L, gi.CONFIG_SEED + 0, 0.59)
+    ref, n, theta, F, thh, Fh = oracle.fix(L, U, ALPHA, 1e-12, 5000)
+    gf = _fixer(L, lgf.LGF_F64, lgf.LGF_REAL18, U)
+    r = gf.fix(ALPHA, 1e-12, 5000)
+    assert r.iterations == n and r.converged
+    assert abs(r.theta - theta) <= 1e-10 * theta
+    assert abs(r.F - F) <= 1e-10 * F
+    assert np.max(np.abs(_cplx(gf.store()) - ref)) <= 1e-11
+    gf.close()
+
+
+def test_config1_convergence_16x4_fp64_12_and_pure_gauge():
+    """configs[1]: 16^4 fp64 12-real to theta < 1e-15; pure-gauge copy of the unit field reaches F = 1."""
+    L = (16, 16, 16, 16)
+    U = gi.make_config(L, gi.CONFIG_SEED + 1, 0.59)
+    ref, n, theta, F, thh, Fh = oracle.fix(L, U, ALPHA, 1e-15, 5000)
+    gf = _fixer(L, lgf.LGF_F64, lgf.LGF_REAL12, U)
+    r = gf.fix(ALPHA, 1e-15, 5000)
+    assert r.iterations == n and r.converged
+    assert abs(r.theta - theta) <= 1e-10 * theta
+    assert abs(r.F - F) <= 1e-10 * F
+    Up = gi.make_config(L, gi.CONFIG_SEED + 1, kind="pure_gauge")
+    _, n2, th2, F2, _, _ = oracle.fix(L, Up, ALPHA, 1e-15, 5000)
+    gf.load(gi.as_real(Up))
+    r2 = gf.fix(ALPHA, 1e-15, 5000)
+    assert r2.iterations == n2 and r2.converged
+    assert abs(1 - r2.F) < 1e-13 and abs(r2.F - F2) < 1e-13
+    gf.close()
+
+
+@pytest.mark.parametrize("L", [(8, 8, 8, 8), (6, 4, 12, 8), (16, 8, 4, 12)])
+@pytest.mark.parametrize("stor", [lgf.LGF_REAL18, lgf.LGF_REAL12])
+def test_fp32_iterations(L, stor):
+    """fp32: generate in fp64, round once, feed the same rounded values to both sides."""
+    U = gi.make_config(L, 25, 0.59)
+    U32 = gi.as_real(U, torch.float32)
+    Ur = gi.from_real(U32)
+    gf = lgf.GaugeFixer(L, lgf.LGF_F32, stor)
+    gf.load(U32)
+    cur = Ur
+    for it in range(1, 4):
+        ref, thh, Fh = oracle.iterate(L, Ur, it, ALPHA)
+        r = gf.iterate(1, ALPHA)
+        got = _cplx(gf.store())
+        assert np.max(np.abs(got - ref)) <= 2e-5
+        assert abs(r.F - Fh[it]) <= 1e-5 * abs(Fh[it])
+    gf.close()
+
+
+@pytest.mark.parametrize("prec", [lgf.LGF_F64, lgf.LGF_F32])
+def test_load_store_roundtrip(prec):
+    L = (6, 4, 12, 8)
+    dt = torch.float64 if prec == lgf.LGF_F64 else torch.float32
+    U = gi.as_real(gi.make_config(L, 26, 0.59), dt)
+    gf = lgf.GaugeFixer(L, prec, lgf.LGF_REAL18)
+    gf.load(U)
+    assert torch.equal(gf.store(), U)                                  # bitwise for 18-real
+    assert torch.equal(gf.store(device="cuda").cpu(), U)
+    gf.load(U.cuda())
+    assert torch.equal(gf.store(), U)
+    gf.close()
+    gf = lgf.GaugeFixer(L, prec, lgf.LGF_REAL12)
+    gf.load(U)
+    out = gf.store()
+    assert torch.equal(out[:, :, :2], U[:, :, :2])                     # rows 0,1 bitwise
+    if prec == lgf.LGF_F64:
+        ref = oracle.two_row_roundtrip(U)
+        assert np.max(np.abs(_cplx(out) - ref)) <= 4e-16
+    else:
+        assert float((out - U).abs().max()) < 1e-6
+    gf.close()
+
+
+def test_fix_semantics_and_errors():
+    L = (4, 4, 4, 4)
+    U = gi.make_config(L, 27, 0.59)
+    gf = lgf.GaugeFixer(L, lgf.LGF_F64, lgf.LGF_REAL18)
+    with pytest.raises(lgf.LgfError):
+        gf.measure()                                                   # LGF_ESTATE before load
+    gf.load(gi.as_real(U))
+    r0 = gf.measure()
+    r = gf.fix(ALPHA, 1e30, 100)                                       # already below tol
+    assert r.iterations == 0 and r.converged and r.theta == r0.theta
+    r = gf.fix(ALPHA, 1e-30, 7)                                        # hits max_iter
+    assert r.iterations == 7 and not r.converged
+    ref, thh, Fh = oracle.iterate(L, U, 7, ALPHA)
+    assert abs(r.theta - thh[7]) <= 1e-10 * thh[7]
+    r = gf.iterate(0, ALPHA)
+    assert r.iterations == 0 and abs(r.theta - thh[7]) <= 1e-10 * thh[7]
+    with pytest.raises(lgf.LgfError):
+        gf.iterate(1, -1.0)
+    with pytest.raises(lgf.LgfError):
+        lgf.GaugeFixer((5, 4, 4, 4))                                   # prime factor 5
+    gf.close()
+
+
+def test_run_to_run_determinism():
+    L = (8, 8, 8, 8)
+    U = gi.as_real(gi.make_config(L, 28, 0.59))
+    outs = []
+    for _ in range(2):
+        gf = lgf.GaugeFixer(L, lgf.LGF_F64, lgf.LGF_REAL12)
+        gf.load(U)
+        r = gf.iterate(10, ALPHA)
+        outs.append((r.theta, r.F, gf.store()))
+        gf.close()
+    assert outs[0][0] == outs[1][0] and outs[0][1] == outs[1][1] and torch.equal(outs[0][2], outs[1][2])
