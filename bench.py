@@ -1,0 +1,343 @@
+#!/usr/bin/env python
+"""bench.py -- gauge-fix iterations/s and achieved HBM GB/s (BASELINE.json `metric`) on one B200.
+
+A "step" is one pass of the whole hot path = ONE gauge-fixing iteration (K2 fft_xy_fwd, K3
+fft_zt_fwd_scale_inv, K4 fft_xy_inv, K5 gbuild_update, K1 delta_theta_F) over one
+synthetic lattice.  Default workload: configs[2], 32^4 SU(3), rough links at mean plaquette 0.59 +
+Haar gauge transform, alpha = 0.08; headline mode fp64 / 12-real (the paper's best variant,
+PAPER.md:72-74), the other three precision x storage modes are reported in "modes".
+
+  python bench.py --gpus N --steps K --warmup W                 # this repo's CUDA path
+  python bench.py --impl reference --gpus N --steps K --warmup W  # the oracle on the host cores
+
+N > 1 (torchrun): "replicas only" -- every rank fixes its own lattice, no data-path collective
+(SURVEY.md §8(e)); value = N*K iterations / max-over-ranks device time.
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import subprocess
+import sys
+import tempfile
+import time
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+if ROOT not in sys.path:
+    sys.path.insert(0, ROOT)
+
+ALPHA = 0.08
+FALLBACK_HBM_GBS = 6650.0          # /opt/skills/guides/B200_PROFILING.md fallback
+
+
+def parse_args():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=1000)
+    ap.add_argument("--warmup", type=int, default=10)
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--lattice", default="32,32,32,32", help="Lx,Ly,Lz,Lt")
+    ap.add_argument("--precision", default="f64", choices=["f64", "f32"])
+    ap.add_argument("--storage", type=int, default=12, choices=[12, 18])
+    ap.add_argument("--modes", default="all", choices=["all", "primary"],
+                    help="all: also time the other three precision/storage modes")
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--no-e2e", action="store_true")
+    ap.add_argument("--plaquette", type=float, default=0.59)
+    return ap.parse_args()
+
+
+def bytes_per_site(kernel: str, n_l: int, w: int) -> int:
+    """Algorithmic bytes per site."""
+    if kernel.startswith("K1"):
+        return (4 * n_l + 8) * w
+    if kernel.startswith("K5"):
+        return (8 * n_l + 8) * w
+    return 16 * w                      # K2, K3, K4: read + write the 8-real packed Delta
+
+
+def measured_peak():
+    try:
+        p = json.load(open(os.path.join(ROOT, "MEASURED_PEAKS.json")))
+        return float(p["hbm_gbs"]), "measured (MEASURED_PEAKS.json hbm_gbs, copy read+write)"
+    except Exception:
+        return FALLBACK_HBM_GBS, "fallback (B200_PROFILING.md 6.65 TB/s)"
+
+
+def ncu_traffic(mode_key: str, kernel: str):
+    """dram bytes per launch from the committed ncu --set full capture, or None."""
+    try:
+        t = json.load(open(os.path.join(ROOT, "profiles", "ncu_traffic.json")))
+        return t.get(mode_key, {}).get(kernel)
+    except Exception:
+        return None
+
+
+class ClockSampler:
+    Q = ("clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.hw_slowdown,"
+         "clocks_event_reasons.hw_thermal_slowdown,clocks_event_reasons.sw_thermal_slowdown,"
+         "clocks_event_reasons.sw_power_cap")
+
+    def __init__(self, index: int):
+        self.f = tempfile.NamedTemporaryFile("w+", suffix=".csv", delete=False)
+        self.p = None
+        try:
+            self.p = subprocess.Popen(["nvidia-smi", "-i", str(index), f"--query-gpu={self.Q}",
+                                       "--format=csv,noheader,nounits", "-lms", "100"],
+                                      stdout=self.f, stderr=subprocess.DEVNULL)
+        except Exception:
+            self.p = None
+
+    def stop(self):
+        out = {"sm_mhz": None, "sm_max_mhz": None, "reasons": []}
+        if self.p is None:
+            return out
+        self.p.terminate()
+        try:
+            self.p.wait(timeout=5)
+        except Exception:
+            self.p.kill()
+        self.f.flush()
+        self.f.seek(0)
+        sm, reasons, smax, pw = [], set(), None, []
+        names = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
+        for line in self.f.read().splitlines():
+            parts = [x.strip() for x in line.split(",")]
+            if len(parts) < 7:
+                continue
+            try:
+                sm.append(float(parts[0]))
+                smax = float(parts[1])
+                pw.append(float(parts[2]))
+            except ValueError:
+                continue
+            for n, v in zip(names, parts[3:7]):
+                if v.lower().startswith("active"):
+                    reasons.add(n)
+        try:
+            os.unlink(self.f.name)
+        except OSError:
+            pass
+        if sm:
+            sm.sort()
+            # median of the upper half = clocks under load (idle samples before/after are low)
+            hi = sm[len(sm) // 2:]
+            out["sm_mhz"] = hi[len(hi) // 2]
+            out["samples"] = len(sm)
+            out["power_w_max"] = max(pw) if pw else None
+        out["sm_max_mhz"] = smax
+        out["reasons"] = sorted(reasons)
+        return out
+
+
+def time_oracle(L, U_real, iters: int):
+    """The oracle as it stands, timed on the host cores: `iters` iterations (each with its
+    measurement) on the given links.  Returns (seconds, threads)."""
+    import oracle
+    oracle.lib()
+    t0 = time.perf_counter()
+    oracle.iterate(L, U_real, iters, ALPHA)
+    return time.perf_counter() - t0, oracle.threads()
+
+
+def run_reference(args, L):
+    """--impl reference: the oracle (unmodified, as it stands) on the box's host cores, same
+    config / metric / unit; each step = one oracle iteration on the same 32^4-shaped workload."""
+    rank = int(os.environ.get("RANK", "0"))
+    if rank != 0:
+        return
+    import torch
+    import lgf_inputs as gi
+    V = gi.volume(L)
+    dev = "cuda" if torch.cuda.is_available() else "cpu"
+    U = gi.make_config(L, gi.CONFIG_SEED + 2, args.plaquette, device=dev).cpu()
+    Ur = gi.as_real(U)
+    steps = max(1, min(args.steps, 3))         # bounded sample: a few iterations of the full lattice
+    warm = min(args.warmup, 1)
+    if warm:
+        time_oracle(L, Ur, 1)
+    sec, thr = time_oracle(L, Ur, steps)
+    # oracle.iterate does 1 initial measurement + steps x (update + measurement)
+    val = steps / sec
+    line = {
+        "impl": "reference", "metric": "gauge_fix_iterations_per_s", "value": val, "unit": "iterations/s",
+        "n_gpus": args.gpus, "steps": steps, "warmup": warm, "ms_per_step": 1e3 * sec / steps,
+        "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+        "config": {"workload": f"{'x'.join(map(str, L))} SU(3), plaquette {args.plaquette}, alpha {ALPHA}",
+                   "sites": V, "note": "oracle/lgf_oracle.cpp (plain C++, OpenMP over sites/lines) on host cores"},
+        "cpu_baseline": {"value": val, "unit": "iterations/s", "cores": thr, "kind": "oracle",
+                         "sample": f"{steps} full iterations of the {'x'.join(map(str, L))} lattice"},
+        "e2e": {"value": val, "unit": "iterations/s", "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+        "gpu_launches": 0,
+    }
+    print(json.dumps(line), flush=True)
+
+
+def main():
+    args = parse_args()
+    L = tuple(int(x) for x in args.lattice.split(","))
+    if args.impl == "reference":
+        run_reference(args, L)
+        return
+
+    import torch
+    import torch.distributed as dist
+    import lgf_inputs as gi
+    import paper_1208_1186_b200 as lgf
+
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    rank = int(os.environ.get("RANK", "0"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py needs a CUDA device: the lgf library has no CPU fallback")
+    torch.cuda.set_device(local)
+    dev = torch.device("cuda", local)
+    if world > 1:
+        dist.init_process_group("nccl", device_id=dev)
+
+    V = gi.volume(L)
+    K, W = args.steps, max(args.warmup, 3)
+    peak, peak_src = measured_peak()
+
+    # every rank: its own seeded lattice (replicas only)
+    U = gi.make_config(L, gi.CONFIG_SEED + 2 + 1000 * rank, args.plaquette, device=dev)
+    plaq = gi.mean_plaquette(U, L)
+
+    primary = (args.precision, args.storage)
+    modes = [primary]
+    if args.modes == "all":
+        modes += [m for m in [("f64", 18), ("f64", 12), ("f32", 18), ("f32", 12)] if m != primary]
+
+    def barrier():
+        if world > 1:
+            dist.barrier()
+        torch.cuda.synchronize()
+
+    results = {}
+    clocks = None
+    total_launches = 0
+    for (prec, stor) in modes:
+        dt = torch.float64 if prec == "f64" else torch.float32
+        gf = lgf.GaugeFixer(L, lgf.LGF_F64 if prec == "f64" else lgf.LGF_F32, stor, device=str(dev))
+        Ud = gi.as_real(U, dt)                       # device tensor: inputs resident in HBM
+        gf.load(Ud)
+        del Ud
+        gf.iterate(W, ALPHA)                         # warm-up (also captures the graph)
+        stream = torch.cuda.current_stream(dev)
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        sampler = ClockSampler(local) if (prec, stor) == primary and rank == 0 else None
+        barrier()
+        n0 = gf.launch_count()
+        e0.record(stream)
+        gf.iterate_async(K, ALPHA)
+        e1.record(stream)
+        res = gf.wait()
+        barrier()
+        launches = gf.launch_count() - n0
+        ms = e0.elapsed_time(e1)
+        if sampler:
+            clocks = sampler.stop()
+        if world > 1:
+            t = torch.tensor([ms], device=dev, dtype=torch.float64)
+            dist.all_reduce(t, op=dist.ReduceOp.MAX)
+            ms = float(t.item())
+        kern_ms, _ = gf.profile_iterate(20, ALPHA)
+        w = 8 if prec == "f64" else 4
+        b_iter = (12 * stor + 64) * w
+        kernels = {}
+        for k, t_ms in kern_ms.items():
+            b = bytes_per_site(k, stor, w) * V
+            kernels[k] = {"ms": t_ms, "algorithmic_GBps": b / (t_ms * 1e-3) / 1e9,
+                          "frac_of_peak": b / (t_ms * 1e-3) / 1e9 / peak,
+                          "share_of_iteration": t_ms / sum(kern_ms.values())}
+        results[(prec, stor)] = {
+            "iterations_per_s": world * K / (ms * 1e-3), "ms_per_iteration": ms / K,
+            "site_updates_per_s": world * K * V / (ms * 1e-3),
+            "algorithmic_GBps": b_iter * V * K / (ms * 1e-3) / 1e9,
+            "frac_of_hbm_peak": b_iter * V * K / (ms * 1e-3) / 1e9 / peak,
+            "bytes_per_site_iteration": b_iter, "theta": res.theta, "F": res.F,
+            "launches": launches, "kernels": kernels,
+        }
+        if (prec, stor) == primary:
+            total_launches = launches
+        gf.close()
+        del gf
+        torch.cuda.empty_cache()
+
+    # ---- e2e: the user's call sequence with HOST buffers: load (H2D) + fix/iterate + store (D2H) ----
+    e2e = None
+    if not args.no_e2e:
+        prec, stor = primary
+        dt = torch.float64 if prec == "f64" else torch.float32
+        host_in = gi.as_real(U, dt).cpu().pin_memory()
+        host_out = torch.empty_like(host_in).pin_memory()
+        gf = lgf.GaugeFixer(L, lgf.LGF_F64 if prec == "f64" else lgf.LGF_F32, stor, device=str(dev))
+        gf.load(host_in)
+        gf.iterate(W, ALPHA)
+        barrier()
+        t0 = time.perf_counter()
+        gf.load(host_in)
+        if prec == "f64":
+            r = gf.fix(ALPHA, 1e-15, 5000)
+        else:
+            r = gf.iterate(50, ALPHA)
+        gf.store(host_out)
+        torch.cuda.synchronize()
+        sec = time.perf_counter() - t0
+        if world > 1:
+            t = torch.tensor([sec], device=dev, dtype=torch.float64)
+            dist.all_reduce(t, op=dist.ReduceOp.MAX)
+            sec = float(t.item())
+        nb = host_in.numel() * host_in.element_size()
+        e2e = {"value": world * r.iterations / sec, "unit": "iterations/s",
+               "h2d_bytes_per_step": nb / max(r.iterations, 1), "d2h_bytes_per_step": nb / max(r.iterations, 1),
+               "job": f"lgf_load(host pinned) + {'lgf_fix(theta<1e-15)' if prec == 'f64' else 'lgf_iterate(50)'} + lgf_store(host)",
+               "iterations": r.iterations, "seconds": sec, "theta": r.theta, "F": r.F,
+               "h2d_bytes": nb, "d2h_bytes": nb}
+        gf.close()
+        del gf, host_in, host_out
+
+    # ---- CPU baseline: the oracle, bounded sample, rank 0 at N = 1 only ----
+    cpu = None
+    if rank == 0 and world == 1 and not args.no_cpu_baseline:
+        iters = 3 if V <= (1 << 20) else 1
+        sec, thr = time_oracle(L, gi.as_real(U).cpu(), iters)
+        cpu = {"value": iters / sec, "unit": "iterations/s", "cores": thr, "kind": "oracle",
+               "sample": f"{iters} full iterations of the same {'x'.join(map(str, L))} lattice ({sec:.1f} s)"}
+
+    if rank == 0:
+        pr = results[primary]
+        dom = max(pr["kernels"].items(), key=lambda kv: kv[1]["ms"])
+        w = 8 if primary[0] == "f64" else 4
+        dom_bytes = bytes_per_site(dom[0], primary[1], w) * V
+        mode_key = f"{primary[0]}_{primary[1]}"
+        line = {
+            "metric": "gauge_fix_iterations_per_s", "value": pr["iterations_per_s"], "unit": "iterations/s",
+            "n_gpus": world, "steps": K, "warmup": W, "ms_per_step": pr["ms_per_iteration"],
+            "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
+            "dtype": primary[0], "data": "synthetic",
+            "config": {"workload": f"configs[2]-shaped: {'x'.join(map(str, L))} SU(3), {primary[0]}, {primary[1]}-real, "
+                                   f"rough links plaquette {plaq:.4f} + Haar gauge transform, alpha {ALPHA}",
+                       "sites": V, "parallelism": "replicas only" if world > 1 else "1 GPU",
+                       "l2": "inputs larger than L2 (links %.0f MB > 126 MB)" % (4 * primary[1] * V * w / 1e6),
+                       "hbm_peak_GBps": peak, "hbm_peak_source": peak_src},
+            "site_updates_per_s": pr["site_updates_per_s"],
+            "achieved_HBM_GBps_algorithmic": pr["algorithmic_GBps"],
+            "iteration_frac_of_hbm_roofline": pr["frac_of_hbm_peak"],
+            "roofline": {"bound": "hbm", "kernel": dom[0], "achieved": dom[1]["algorithmic_GBps"], "peak": peak,
+                         "unit": "GB/s", "frac": dom[1]["frac_of_peak"], "traffic": ncu_traffic(mode_key, dom[0]),
+                         "algorithmic_bytes_per_launch": dom_bytes, "peak_source": peak_src},
+            "cpu_baseline": cpu,
+            "e2e": e2e,
+            "gpu_launches": total_launches,
+            "clocks": clocks,
+            "modes": {f"{p}_{s}": {k: v for k, v in r.items()} for (p, s), r in results.items()},
+        }
+        print(json.dumps(line), flush=True)
+    if world > 1:
+        dist.destroy_process_group()
+
+
+if __name__ == "__main__":
+    main()

@@ -7,13 +7,12 @@ import subprocess
 _HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(_HERE, "csrc")
 LIB = os.path.join(_HERE, "liblgf.so")
-SOURCES = ["lgf_api.cu"]
-HEADERS = ["lgf_math.cuh", "lgf_site.cuh", "lgf_fft.cuh", os.path.join("..", "..", "include", "lgf.h")]
+SOURCES = ["lgf_api.cu", "lgf_fft_inst.cu", "lgf_fft_inst_f64.cu", "lgf_fft_inst_f32.cu"]
+HEADERS = ["lgf_math.cuh", "lgf_site.cuh", "lgf_fft.cuh", "lgf_regfft.cuh", "lgf_fft_ct.cuh", "lgf_fft_inst.cuh",
+           "lgf_fft_inst_impl.cuh", os.path.join("..", "..", "include", "lgf.h")]
 
-NVCC_FLAGS = [
-    "-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo", "-O3", "-std=c++17",
-    "-Xcompiler", "-fPIC", "-shared", "--cudart", "shared",
-]
+NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo", "-O3", "-std=c++17", "-Xcompiler", "-fPIC"]
+LINK_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-shared", "--cudart", "shared"]
 
 
 def _stale() -> bool:
@@ -25,12 +24,22 @@ def _stale() -> bool:
 
 
 def build(force: bool = False, verbose: bool = False) -> str:
-    """nvcc-compile the library if it is missing or older than its sources.  Needs no GPU."""
+    """nvcc-compile the library if it is missing or older than its sources (translation units in
+    parallel, then one link).  Needs no GPU: nvcc cross-compiles sm_100a."""
     if force or _stale():
         nvcc = os.environ.get("NVCC", "/usr/local/cuda/bin/nvcc")
-        cmd = [nvcc] + NVCC_FLAGS + (["-Xptxas", "-v"] if verbose else []) + \
-              ["-o", LIB + ".tmp"] + [os.path.join(CSRC, f) for f in SOURCES]
-        subprocess.run(cmd, check=True)
+        objdir = os.path.join(_HERE, "build")
+        os.makedirs(objdir, exist_ok=True)
+        procs, objs = [], []
+        for src in SOURCES:
+            obj = os.path.join(objdir, src.replace(".cu", ".o"))
+            objs.append(obj)
+            cmd = [nvcc] + NVCC_FLAGS + (["-Xptxas", "-v"] if verbose else []) + ["-c", "-o", obj, os.path.join(CSRC, src)]
+            procs.append((src, subprocess.Popen(cmd)))
+        for src, p in procs:
+            if p.wait() != 0:
+                raise RuntimeError(f"nvcc failed on {src}")
+        subprocess.run([nvcc] + LINK_FLAGS + ["-o", LIB + ".tmp"] + objs, check=True)
         os.replace(LIB + ".tmp", LIB)
     return LIB
 

@@ -34,7 +34,8 @@ class LgfResult:
 
 
 def library_path() -> str:
-    return os.path.join(_HERE, "liblgf.so")
+    # LGF_LIBRARY: developer override used to A/B kernel variants; the default is the in-tree build
+    return os.environ.get("LGF_LIBRARY") or os.path.join(_HERE, "liblgf.so")
 
 
 def declared_symbols() -> list:

@@ -6,11 +6,14 @@
 
 #include <cmath>
 #include <cstdio>
+#include <cstdlib>
 #include <cstring>
 #include <new>
 #include <vector>
 
 #include "lgf_fft.cuh"
+#include "lgf_fft_ct.cuh"
+#include "lgf_fft_inst.cuh"
 #include "lgf_site.cuh"
 
 using namespace lgf;
@@ -106,6 +109,11 @@ struct lgf_ctx {
     ZtPass zt;                   // K3
     int xy_threads, zt_threads;
     size_t xy_smem, zt_smem;
+    // compile-time-sized fast path (nullptr: generic kernels above)
+    const XyCtEntry* xy_ct;
+    const ZtCtEntry* zt_ct;
+    XyArgs xy_args;
+    ZtArgs zt_args;
     bool loaded, delta_valid;
     int64_t launches;
     // iteration graph (K2 K3 K4 K5 K1), captured per alpha
@@ -198,6 +206,31 @@ bool plan_passes(lgf_ctx* c) {
     Z.scale_num = pmax / (double)c->V;
     c->zt_threads = threads_for(best * LzLt, c->axis[2], c->axis[3]);
     c->zt_smem = (size_t)Z.pt * L[3] * cb;
+    // fast path: both passes must be available, because K2's compile-time kernels leave the (x,y)
+    // spectrum in digit-swapped order, which only the compile-time K3 knows how to un-swap
+    c->zt_ct = find_zt_ct(c->precision, L[2], L[3], LxLy);
+    c->xy_ct = c->zt_ct ? find_xy_ct(c->precision, L[0], L[1]) : nullptr;
+    if (getenv("LGF_FORCE_GENERIC_FFT")) c->xy_ct = nullptr, c->zt_ct = nullptr;
+    if (c->xy_ct) {
+        c->xy_args.twx_fwd = c->axis[0].tw_fwd; c->xy_args.twx_inv = c->axis[0].tw_inv;
+        c->xy_args.twy_fwd = c->axis[1].tw_fwd; c->xy_args.twy_inv = c->axis[1].tw_inv;
+        c->xy_args.nplanes = (int)(4 * LzLt);
+    }
+    if (c->zt_ct) {
+        ZtArgs& A = c->zt_args;
+        A.twz_fwd = c->axis[2].tw_fwd; A.twz_inv = c->axis[2].tw_inv;
+        A.twt_fwd = c->axis[3].tw_fwd; A.twt_inv = c->axis[3].tw_inv;
+        A.psq_x = c->axis[0].psq; A.psq_y = c->axis[1].psq; A.psq_z = c->axis[2].psq; A.psq_t = c->axis[3].psq;
+        A.V = c->V;
+        A.LxLy = LxLy;
+        A.Lx = L[0];
+        A.tiles_per_comp = (int)(LxLy / c->zt_ct->cx);
+        A.scale_num = Z.scale_num;
+        A.x_n1 = c->xy_ct ? c->xy_ct->x_n1 : L[0];
+        A.x_n2 = L[0] / A.x_n1;
+        A.y_n1 = c->xy_ct ? c->xy_ct->y_n1 : L[1];
+        A.y_n2 = L[1] / A.y_n1;
+    }
     return true;
 }
 
@@ -247,6 +280,21 @@ struct Impl {
     static int fft(lgf_ctx* c, int k, bool gated) {
         const int* done = gated ? &dev_state(c)->done : nullptr;
         const unsigned planes = (unsigned)(4 * (long long)c->L[2] * c->L[3]);
+        Cx<T>* dptr = delta(c);
+        if (k != 1 && c->xy_ct) {
+            const XyCtEntry* e = c->xy_ct;
+            void* args[] = {&dptr, &c->xy_args, &done};
+            CU(cudaLaunchKernel(k == 0 ? e->k_fwd : e->k_inv, dim3((planes + e->pb - 1) / e->pb), dim3(e->threads), args, e->smem, c->stream));
+            c->launches++;
+            return LGF_OK;
+        }
+        if (k == 1 && c->zt_ct) {
+            const ZtCtEntry* e = c->zt_ct;
+            void* args[] = {&dptr, &c->zt_args, &done};
+            CU(cudaLaunchKernel(e->kernel, dim3(4 * c->zt_args.tiles_per_comp), dim3(e->threads), args, e->smem, c->stream));
+            c->launches++;
+            return LGF_OK;
+        }
         if (k == 0)
             fft_xy_kernel<T, -1><<<planes, c->xy_threads, c->xy_smem, c->stream>>>(delta(c), c->xy, done);
         else if (k == 2)
@@ -261,6 +309,7 @@ struct Impl {
         CU(cudaFuncSetAttribute(fft_xy_kernel<T, -1>, cudaFuncAttributeMaxDynamicSharedMemorySize, kMaxSmem));
         CU(cudaFuncSetAttribute(fft_xy_kernel<T, +1>, cudaFuncAttributeMaxDynamicSharedMemorySize, kMaxSmem));
         CU(cudaFuncSetAttribute(fft_zt_kernel<T>, cudaFuncAttributeMaxDynamicSharedMemorySize, kMaxSmem));
+        CU(prepare_ct_kernels(c->precision));
         return upload_tables<T>(c);
     }
     static int load(lgf_ctx* c, const void* src, int memspace) {

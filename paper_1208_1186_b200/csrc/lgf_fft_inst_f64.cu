@@ -1,0 +1,31 @@
+// fp64 instantiations of the compile-time-sized FFT kernels.  N1 = N means "whole line in
+// registers"; 48 = 8*6 and 64 = 8*8 are split in two register stages.
+#include "lgf_fft_inst_impl.cuh"
+
+namespace lgf {
+using namespace inst;
+typedef double T;
+
+const XyCtEntry* xy_table_f64(int* n) {
+    static const XyCtEntry tab[] = {
+        XyInst<T, 8, 8, 8, 8, 16>::entry(),
+        XyInst<T, 16, 16, 16, 16, 8>::entry(),
+        XyInst<T, 32, 32, 32, 32, 4>::entry(),
+        XyInst<T, 48, 8, 48, 8, 1>::entry(),
+        XyInst<T, 64, 8, 64, 8, 1>::entry(),
+    };
+    *n = (int)(sizeof(tab) / sizeof(tab[0]));
+    return tab;
+}
+const ZtCtEntry* zt_table_f64(int* n) {
+    static const ZtCtEntry tab[] = {
+        ZtInst<T, 8, 8, 8, 8, 4>::entry(),
+        ZtInst<T, 16, 16, 16, 16, 4>::entry(),
+        ZtInst<T, 32, 32, 32, 32, 4>::entry(),
+        ZtInst<T, 48, 8, 8, 8, 4>::entry(),
+        ZtInst<T, 64, 8, 64, 8, 2>::entry(),
+    };
+    *n = (int)(sizeof(tab) / sizeof(tab[0]));
+    return tab;
+}
+}  // namespace lgf

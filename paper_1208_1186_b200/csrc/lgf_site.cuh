@@ -8,6 +8,10 @@
 #pragma once
 #include "lgf_math.cuh"
 
+#ifndef LGF_SITE_MINB
+#define LGF_SITE_MINB 2     // resident CTAs per SM the site kernels are compiled for (register cap)
+#endif
+
 namespace lgf {
 
 struct Geom {
@@ -95,7 +99,7 @@ __device__ __forceinline__ void block_sum2(double& a, double& b) {
 // evaluates the stopping test theta < tol / iter >= max_iter on the device).
 // ---------------------------------------------------------------------------------------------
 template <typename T, int NC, class Tile>
-__global__ void __launch_bounds__(Tile::kThreads)
+__global__ void __launch_bounds__(Tile::kThreads, LGF_SITE_MINB)
 k1_delta_theta_F(const Cx<T>* __restrict__ U, Cx<T>* __restrict__ D, double2* __restrict__ partials,
                  DevState* st, Geom g, int mode) {
     if (mode == 1 && *reinterpret_cast<volatile int*>(&st->done)) return;
@@ -181,7 +185,7 @@ __device__ __forceinline__ void load_g(Su3<T>& g, const Cx<T>* __restrict__ D, l
 }
 
 template <typename T, int NC, class Tile>
-__global__ void __launch_bounds__(Tile::kThreads)
+__global__ void __launch_bounds__(Tile::kThreads, LGF_SITE_MINB)
 k5_gbuild_update(Cx<T>* __restrict__ U, const Cx<T>* __restrict__ D, const DevState* st, Geom g, T half_alpha) {
     if (*reinterpret_cast<const volatile int*>(&st->done)) return;
     int x[4];

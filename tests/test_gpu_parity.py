@@ -12,7 +12,9 @@ import paper_1208_1186_b200 as lgf
 pytestmark = pytest.mark.gpu
 ALPHA = 0.08
 
-SHAPES = [(8, 8, 8, 8), (6, 4, 12, 8), (4, 6, 3, 2), (16, 8, 4, 12), (12, 12, 6, 4), (2, 2, 2, 2), (24, 18, 4, 8)]
+# compile-time-sized FFT kernels: (8,8,8,8), (16,16,8,8), (16,16,16,16); mixed / generic runtime-radix kernels: the rest
+SHAPES = [(8, 8, 8, 8), (16, 16, 8, 8), (6, 4, 12, 8), (4, 6, 3, 2), (16, 8, 4, 12), (12, 12, 6, 4), (2, 2, 2, 2),
+          (24, 18, 4, 8), (8, 8, 16, 16)]
 MODES = [(lgf.LGF_F64, lgf.LGF_REAL18), (lgf.LGF_F64, lgf.LGF_REAL12)]
 
 
@@ -205,3 +207,49 @@ def test_run_to_run_determinism():
         outs.append((r.theta, r.F, gf.store()))
         gf.close()
     assert outs[0][0] == outs[1][0] and outs[0][1] == outs[1][1] and torch.equal(outs[0][2], outs[1][2])
+
+
+@pytest.mark.parametrize("L,prec,stor", [((32, 32, 32, 32), lgf.LGF_F64, lgf.LGF_REAL12),
+                                         ((32, 32, 32, 32), lgf.LGF_F64, lgf.LGF_REAL18),
+                                         ((48, 48, 48, 8), lgf.LGF_F64, lgf.LGF_REAL12)])
+def test_full_size_one_iteration(L, prec, stor):
+    """BASELINE.json's full sizes (configs[2], configs[3]) in the launch configuration bench.py times:
+    every link after one iteration against the oracle, element by element."""
+    U = gi.make_config(L, gi.CONFIG_SEED + 2, 0.59, device="cuda").cpu()
+    ref, thh, Fh = oracle.iterate(L, U, 1, ALPHA)
+    gf = _fixer(L, prec, stor, U)
+    r0 = gf.measure()
+    assert abs(r0.theta - thh[0]) <= 1e-12 * thh[0]
+    r = gf.iterate(1, ALPHA)
+    got = _cplx(gf.store())
+    assert np.max(np.abs(got - ref)) <= 1e-12
+    assert abs(r.theta - thh[1]) <= 1e-11 * thh[1] and abs(r.F - Fh[1]) <= 1e-12
+    gf.close()
+
+
+def test_full_size_fp32_32x4():
+    L = (32, 32, 32, 32)
+    U32 = gi.as_real(gi.make_config(L, gi.CONFIG_SEED + 2, 0.59, device="cuda").cpu(), torch.float32)
+    ref, thh, Fh = oracle.iterate(L, gi.from_real(U32), 2, ALPHA)
+    for stor in (lgf.LGF_REAL12, lgf.LGF_REAL18):
+        gf = lgf.GaugeFixer(L, lgf.LGF_F32, stor)
+        gf.load(U32)
+        r = gf.iterate(2, ALPHA)
+        assert np.max(np.abs(_cplx(gf.store()) - ref)) <= 2e-5
+        assert abs(r.F - Fh[2]) <= 1e-5 * abs(Fh[2])
+        gf.close()
+
+
+def test_generic_and_compile_time_fft_paths_agree(monkeypatch):
+    """The runtime-radix kernels (forced by LGF_FORCE_GENERIC_FFT) and the compile-time-sized kernels
+    must both match the oracle on a shape that has both."""
+    L = (16, 16, 8, 8)
+    U = gi.make_config(L, 29, 0.59)
+    ref, thh, _ = oracle.iterate(L, U, 2, ALPHA)
+    for force in (False, True):
+        if force:
+            monkeypatch.setenv("LGF_FORCE_GENERIC_FFT", "1")
+        gf = _fixer(L, lgf.LGF_F64, lgf.LGF_REAL18, U)
+        gf.iterate(2, ALPHA)
+        assert np.max(np.abs(_cplx(gf.store()) - ref)) <= 1e-12
+        gf.close()
