@@ -1,24 +1,41 @@
 // lgf_fft_inst.cu -- lookup over the instantiation tables of the compile-time-sized FFT kernels.
 #include "lgf_fft_inst.cuh"
 
+#include <cstdlib>
+
 namespace lgf {
 
 static const XyCtEntry* xy_tab(int precision, int* n) { return precision ? xy_table_f64(n) : xy_table_f32(n); }
 static const ZtCtEntry* zt_tab(int precision, int* n) { return precision ? zt_table_f64(n) : zt_table_f32(n); }
 
+// Several entries may serve the same extents (different splits / tile sizes): the first one is the
+// tuned default; LGF_XY_VARIANT / LGF_ZT_VARIANT = v select the v-th match (developer A/B knob).
+static int variant(const char* name) {
+    const char* e = getenv(name);
+    return e ? atoi(e) : 0;
+}
+
 const XyCtEntry* find_xy_ct(int precision, int nx, int ny) {
-    int n = 0;
+    int n = 0, skip = variant("LGF_XY_VARIANT");
     const XyCtEntry* t = xy_tab(precision, &n);
+    const XyCtEntry* last = nullptr;
     for (int i = 0; i < n; ++i)
-        if (t[i].nx == nx && t[i].ny == ny) return &t[i];
-    return nullptr;
+        if (t[i].nx == nx && t[i].ny == ny) {
+            last = &t[i];
+            if (skip-- == 0) return last;
+        }
+    return last;
 }
 const ZtCtEntry* find_zt_ct(int precision, int nz, int nt, long long LxLy) {
-    int n = 0;
+    int n = 0, skip = variant("LGF_ZT_VARIANT");
     const ZtCtEntry* t = zt_tab(precision, &n);
+    const ZtCtEntry* last = nullptr;
     for (int i = 0; i < n; ++i)
-        if (t[i].nz == nz && t[i].nt == nt && LxLy % t[i].cx == 0) return &t[i];
-    return nullptr;
+        if (t[i].nz == nz && t[i].nt == nt && LxLy % t[i].cx == 0) {
+            last = &t[i];
+            if (skip-- == 0) return last;
+        }
+    return last;
 }
 cudaError_t prepare_ct_kernels(int precision) {
     int n = 0;

@@ -11,6 +11,11 @@ const XyCtEntry* xy_table_f64(int* n) {
         XyInst<T, 8, 8, 8, 8, 16>::entry(),
         XyInst<T, 16, 16, 16, 16, 8>::entry(),
         XyInst<T, 32, 32, 32, 32, 4>::entry(),
+        XyInst<T, 32, 32, 32, 32, 2>::entry(),
+        XyInst<T, 32, 8, 32, 8, 1>::entry(),
+        XyInst<T, 32, 8, 32, 8, 2>::entry(),
+        XyInst<T, 32, 16, 32, 16, 2>::entry(),
+        XyInst<T, 32, 32, 32, 32, 8>::entry(),
         XyInst<T, 48, 8, 48, 8, 1>::entry(),
         XyInst<T, 64, 8, 64, 8, 1>::entry(),
     };
@@ -22,6 +27,12 @@ const ZtCtEntry* zt_table_f64(int* n) {
         ZtInst<T, 8, 8, 8, 8, 4>::entry(),
         ZtInst<T, 16, 16, 16, 16, 4>::entry(),
         ZtInst<T, 32, 32, 32, 32, 4>::entry(),
+        ZtInst<T, 32, 32, 32, 32, 2>::entry(),
+        ZtInst<T, 32, 8, 32, 8, 4>::entry(),
+        ZtInst<T, 32, 8, 32, 8, 2>::entry(),
+        ZtInst<T, 32, 16, 32, 16, 4>::entry(),
+        ZtInst<T, 32, 8, 32, 32, 4>::entry(),
+        ZtInst<T, 32, 32, 32, 8, 4>::entry(),
         ZtInst<T, 48, 8, 8, 8, 4>::entry(),
         ZtInst<T, 64, 8, 64, 8, 2>::entry(),
     };
