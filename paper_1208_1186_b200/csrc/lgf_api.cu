@@ -15,6 +15,7 @@
 #include "lgf_fft_ct.cuh"
 #include "lgf_fft_inst.cuh"
 #include "lgf_site.cuh"
+#include "lgf_site_mu.cuh"
 
 using namespace lgf;
 
@@ -35,7 +36,21 @@ int cuda_fail(cudaError_t e, const char* what) {
 constexpr size_t kAlign = 256;
 size_t align_up(size_t v) { return (v + kAlign - 1) / kAlign * kAlign; }
 
-typedef SiteTile<8, 4, 4, 2> TileA;
+// thread-per-site tilings (256 sites each); wider x = longer contiguous runs per link plane
+typedef SiteTile<8, 4, 4, 2> Tile0;
+typedef SiteTile<16, 4, 2, 2> Tile1;
+typedef SiteTile<32, 2, 2, 2> Tile2;
+typedef SiteTile<16, 2, 4, 2> Tile3;
+typedef SiteTile<32, 4, 2, 1> Tile4;
+typedef SiteTile<32, 2, 4, 1> Tile5;
+constexpr int kNumSiteTiles = 6;
+const int kSiteTileDims[kNumSiteTiles][4] = {{8, 4, 4, 2}, {16, 4, 2, 2}, {32, 2, 2, 2}, {16, 2, 4, 2}, {32, 4, 2, 1}, {32, 2, 4, 1}};
+// (site, direction) tilings of k5m: 64 sites x 4 directions
+typedef SiteTileMu<8, 4, 2, 1> TileM0;
+typedef SiteTileMu<32, 2, 1, 1> TileM1;
+typedef SiteTileMu<16, 4, 1, 1> TileM2;
+constexpr int kNumMuTiles = 3;
+const int kMuTileDims[kNumMuTiles][4] = {{8, 4, 2, 1}, {32, 2, 1, 1}, {16, 4, 1, 1}};
 constexpr int kStageSites = 1 << 15;       // boundary staging chunk (sites)
 constexpr int kMaxSmem = 200 * 1024;       // per-CTA dynamic shared memory we are willing to ask for
 constexpr int kFixBatch = 8;               // iterations enqueued per polling batch in lgf_fix
@@ -58,6 +73,8 @@ struct Layout {          // byte offsets into the workspace
     size_t state, partials, tw[4], twi[4], psq[4], links, delta, staging, total;
     int nblocks_site;
     int nb[4];
+    int nblocks_mu;          // tiling of the (site, direction) kernels
+    int nbm[4];
 };
 
 bool valid_args(const int32_t L[4], int precision, int storage) {
@@ -73,10 +90,16 @@ Layout make_layout(const int32_t L[4], int precision, int storage) {
     Layout lo;
     const size_t w = precision == LGF_F64 ? 8 : 4;
     const size_t V = (size_t)L[0] * L[1] * L[2] * L[3];
-    const int tile[4] = {8, 4, 4, 2};
-    size_t nb = 1;
-    for (int i = 0; i < 4; ++i) { lo.nb[i] = (L[i] + tile[i] - 1) / tile[i]; nb *= lo.nb[i]; }
-    lo.nblocks_site = (int)nb;
+    size_t nb = 0;                 // most CTAs any thread-per-site tiling needs (sizes the partials)
+    for (int t = 0; t < kNumSiteTiles; ++t) {
+        size_t n = 1;
+        for (int i = 0; i < 4; ++i) n *= (size_t)((L[i] + kSiteTileDims[t][i] - 1) / kSiteTileDims[t][i]);
+        if (n > nb) nb = n;
+    }
+    for (int i = 0; i < 4; ++i) lo.nb[i] = 0;
+    lo.nblocks_site = 0;           // set by choose_site_tile()
+    for (int i = 0; i < 4; ++i) lo.nbm[i] = 0;
+    lo.nblocks_mu = 0;             // set at create
     size_t off = 0;
     lo.state = off; off += align_up(sizeof(DevState));
     lo.partials = off; off += align_up(nb * sizeof(double2));
@@ -104,6 +127,10 @@ struct lgf_ctx {
     cudaStream_t cap_stream;     // library-owned stream used only to CAPTURE graphs (the legacy default stream cannot be captured)
     Layout lo;
     Geom geom;
+    Geom geom_mu;                // tiling of the (site, direction) kernels
+    int site_variant;            // 0: thread per (site, direction); 1: thread per site
+    int site_tile;               // index into kSiteTileDims for the thread-per-site kernels
+    int mu_tile;                 // index into kMuTileDims for k5m
     Axis axis[4];
     XyPass xy;                   // K2, K4
     ZtPass zt;                   // K3
@@ -264,15 +291,47 @@ struct Impl {
     static Cx<T>* staging(lgf_ctx* c) { return reinterpret_cast<Cx<T>*>(c->ws + c->lo.staging); }
 
     static int k1(lgf_ctx* c, int mode) {
-        k1_delta_theta_F<T, NC, TileA><<<c->lo.nblocks_site, TileA::kThreads, 0, c->stream>>>(
-            links(c), delta(c), reinterpret_cast<double2*>(c->ws + c->lo.partials), dev_state(c), c->geom, mode);
-        c->launches++;
+        double2* partials = reinterpret_cast<double2*>(c->ws + c->lo.partials);
+        int nblocks;
+        {
+            nblocks = c->lo.nblocks_site;
+#define LGF_K1_CASE(ID, TILE) case ID: k1_delta_theta_F<T, NC, TILE><<<nblocks, TILE::kThreads, 0, c->stream>>>( \
+                links(c), delta(c), partials, dev_state(c), c->geom, mode); break;
+            switch (c->site_tile) {
+                LGF_K1_CASE(1, Tile1) LGF_K1_CASE(2, Tile2) LGF_K1_CASE(3, Tile3) LGF_K1_CASE(4, Tile4) LGF_K1_CASE(5, Tile5)
+                default: k1_delta_theta_F<T, NC, Tile0><<<nblocks, Tile0::kThreads, 0, c->stream>>>(
+                    links(c), delta(c), partials, dev_state(c), c->geom, mode);
+            }
+#undef LGF_K1_CASE
+        }
+        CU(cudaGetLastError());
+        k1_finish<<<1, 256, 0, c->stream>>>(partials, nblocks, dev_state(c), (double)c->V, mode);
+        c->launches += 2;
         CU(cudaGetLastError());
         return LGF_OK;
     }
     static int k5(lgf_ctx* c, double alpha) {
-        k5_gbuild_update<T, NC, TileA><<<c->lo.nblocks_site, TileA::kThreads, 0, c->stream>>>(
-            links(c), delta(c), dev_state(c), c->geom, (T)(0.5 * alpha));
+        if (c->site_variant == 0) {
+#define LGF_K5M_CASE(ID, TILE) case ID: k5m_gbuild_update<T, NC, TILE><<<c->lo.nblocks_mu, TILE::kThreads, 0, c->stream>>>( \
+                links(c), delta(c), dev_state(c), c->geom_mu, (T)(0.5 * alpha)); break;
+            switch (c->mu_tile) {
+                LGF_K5M_CASE(1, TileM1) LGF_K5M_CASE(2, TileM2)
+                default: k5m_gbuild_update<T, NC, TileM0><<<c->lo.nblocks_mu, TileM0::kThreads, 0, c->stream>>>(
+                    links(c), delta(c), dev_state(c), c->geom_mu, (T)(0.5 * alpha));
+            }
+#undef LGF_K5M_CASE
+            c->launches++;
+            CU(cudaGetLastError());
+            return LGF_OK;
+        }
+#define LGF_K5_CASE(ID, TILE) case ID: k5_gbuild_update<T, NC, TILE><<<c->lo.nblocks_site, TILE::kThreads, 0, c->stream>>>( \
+            links(c), delta(c), dev_state(c), c->geom, (T)(0.5 * alpha)); break;
+        switch (c->site_tile) {
+            LGF_K5_CASE(1, Tile1) LGF_K5_CASE(2, Tile2) LGF_K5_CASE(3, Tile3) LGF_K5_CASE(4, Tile4) LGF_K5_CASE(5, Tile5)
+            default: k5_gbuild_update<T, NC, Tile0><<<c->lo.nblocks_site, Tile0::kThreads, 0, c->stream>>>(
+                links(c), delta(c), dev_state(c), c->geom, (T)(0.5 * alpha));
+        }
+#undef LGF_K5_CASE
         c->launches++;
         CU(cudaGetLastError());
         return LGF_OK;
@@ -481,8 +540,32 @@ static int create_common(const int32_t L[4], int precision, int storage, void* w
     c->stream = reinterpret_cast<cudaStream_t>(stream);
     c->lo = make_layout(L, precision, storage);
     c->pending_n = -1;
+    {   // thread-per-site tiling: widest x tile that divides Lx (LGF_SITE_TILE overrides, A/B knob)
+        int t = (L[0] % 32 == 0) ? 4 : ((L[0] % 16 == 0) ? 1 : 0);
+        const char* e = getenv("LGF_SITE_TILE");
+        if (e && atoi(e) >= 0 && atoi(e) < kNumSiteTiles) t = atoi(e);
+        c->site_tile = t;
+        int n = 1;
+        for (int i = 0; i < 4; ++i) { c->lo.nb[i] = (L[i] + kSiteTileDims[t][i] - 1) / kSiteTileDims[t][i]; n *= c->lo.nb[i]; }
+        c->lo.nblocks_site = n;
+    }
     for (int i = 0; i < 4; ++i) { c->geom.L[i] = L[i]; c->geom.nb[i] = c->lo.nb[i]; }
     c->geom.V = c->V;
+    {   // K5 flavour: 0 = thread per (site, direction), 1 = thread per site (LGF_SITE_VARIANT / LGF_SITEMU_TILE: A/B knobs)
+        const char* e = getenv("LGF_SITE_VARIANT");
+        // measured at 32^4: the (site, direction) split wins for fp64 18-real and fp32 12-real
+        const bool mu_default = (precision == LGF_F64 && storage == LGF_REAL18) || (precision == LGF_F32 && storage == LGF_REAL12);
+        c->site_variant = e ? atoi(e) : (mu_default ? 0 : 1);
+        int t = (L[0] % 16 == 0) ? 2 : 0;
+        e = getenv("LGF_SITEMU_TILE");
+        if (e && atoi(e) >= 0 && atoi(e) < kNumMuTiles) t = atoi(e);
+        c->mu_tile = t;
+        int n = 1;
+        for (int i = 0; i < 4; ++i) { c->lo.nbm[i] = (L[i] + kMuTileDims[t][i] - 1) / kMuTileDims[t][i]; n *= c->lo.nbm[i]; }
+        c->lo.nblocks_mu = n;
+    }
+    c->geom_mu = c->geom;
+    for (int i = 0; i < 4; ++i) c->geom_mu.nb[i] = c->lo.nbm[i];
     int rc = LGF_OK;
     if (ws_bytes < c->lo.total || (reinterpret_cast<uintptr_t>(ws) % kAlign) != 0) rc = LGF_EINVAL;
     if (!rc && !plan_passes(c)) rc = LGF_EUNSUPPORTED;

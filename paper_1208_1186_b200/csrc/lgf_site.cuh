@@ -8,9 +8,6 @@
 #pragma once
 #include "lgf_math.cuh"
 
-#ifndef LGF_SITE_MINB
-#define LGF_SITE_MINB 2     // resident CTAs per SM the site kernels are compiled for (register cap)
-#endif
 
 namespace lgf {
 
@@ -29,6 +26,14 @@ struct DevState {
     unsigned int ticket;     // K1 block counter for the last-block reduction
     double tol;
     long long max_iter;
+};
+
+// Resident CTAs per SM each site kernel is compiled for (= register cap 65536 / (256 * n)); measured
+// best of 1..4 per precision and storage at 32^4.
+template <typename T, int NC> struct SiteOcc {
+    static constexpr int k1 = sizeof(T) == 8 ? 2 : 3;
+    static constexpr int k5 = sizeof(T) == 8 ? 2 : (NC == 6 ? 4 : 2);
+    static constexpr int k5m = sizeof(T) == 8 ? 2 : 3;
 };
 
 template <int TX, int TY, int TZ, int TT>
@@ -99,10 +104,10 @@ __device__ __forceinline__ void block_sum2(double& a, double& b) {
 // evaluates the stopping test theta < tol / iter >= max_iter on the device).
 // ---------------------------------------------------------------------------------------------
 template <typename T, int NC, class Tile>
-__global__ void __launch_bounds__(Tile::kThreads, LGF_SITE_MINB)
+__global__ void __launch_bounds__(Tile::kThreads, SiteOcc<T, NC>::k1)
 k1_delta_theta_F(const Cx<T>* __restrict__ U, Cx<T>* __restrict__ D, double2* __restrict__ partials,
-                 DevState* st, Geom g, int mode) {
-    if (mode == 1 && *reinterpret_cast<volatile int*>(&st->done)) return;
+                 const DevState* st, Geom g, int mode) {
+    if (mode == 1 && *reinterpret_cast<const volatile int*>(&st->done)) return;
     int x[4];
     const bool valid = Tile::coords(g, x);
     double th = 0.0, fn = 0.0;
@@ -140,35 +145,32 @@ k1_delta_theta_F(const Cx<T>* __restrict__ U, Cx<T>* __restrict__ D, double2* __
         fn = (double)retr;
     }
     block_sum2<Tile::kThreads>(th, fn);
-    __shared__ bool is_last;
-    if (threadIdx.x == 0) {
-        partials[blockIdx.x] = make_double2(th, fn);
-        __threadfence();
-        const unsigned int t = atomicAdd(&st->ticket, 1u);
-        is_last = (t == gridDim.x - 1);
-    }
-    __syncthreads();
-    if (!is_last) return;
-    __threadfence();
-    // last block: fixed-order sum of all partials (independent of which block came last)
+    if (threadIdx.x == 0) partials[blockIdx.x] = make_double2(th, fn);   // summed by k1_finish
+}
+
+// Second half of K1: one CTA sums the per-CTA (theta, F) partials in index order (deterministic, no
+// float atomics), publishes theta and F and, at the end of an iteration (mode 1), bumps the
+// iteration count and evaluates the stopping test on the device.  A separate tiny launch instead
+// of a last-CTA ticket: the K1 CTAs then retire without a fence + atomic tail.
+__global__ void __launch_bounds__(256)
+k1_finish(const double2* __restrict__ partials, int n, DevState* st, double V, int mode) {
+    if (mode == 1 && *reinterpret_cast<volatile int*>(&st->done)) return;
     double a = 0.0, b = 0.0;
-    for (unsigned int i = threadIdx.x; i < gridDim.x; i += Tile::kThreads) {
-        const double2 p = __ldcg(partials + i);
+    for (int i = threadIdx.x; i < n; i += 256) {
+        const double2 p = partials[i];
         a += p.x;
         b += p.y;
     }
-    block_sum2<Tile::kThreads>(a, b);
+    block_sum2<256>(a, b);
     if (threadIdx.x == 0) {
-        const double theta = a / (3.0 * (double)g.V);
+        const double theta = a / (3.0 * V);
         st->theta = theta;
-        st->F = b / (12.0 * (double)g.V);
-        st->ticket = 0;
+        st->F = b / (12.0 * V);
         if (mode == 1) {
             const long long it = st->iter + 1;
             st->iter = it;
             if (theta < st->tol || it >= st->max_iter) st->done = 1;
         }
-        __threadfence();
     }
 }
 
@@ -185,7 +187,7 @@ __device__ __forceinline__ void load_g(Su3<T>& g, const Cx<T>* __restrict__ D, l
 }
 
 template <typename T, int NC, class Tile>
-__global__ void __launch_bounds__(Tile::kThreads, LGF_SITE_MINB)
+__global__ void __launch_bounds__(Tile::kThreads, SiteOcc<T, NC>::k5)
 k5_gbuild_update(Cx<T>* __restrict__ U, const Cx<T>* __restrict__ D, const DevState* st, Geom g, T half_alpha) {
     if (*reinterpret_cast<const volatile int*>(&st->done)) return;
     int x[4];
