@@ -70,8 +70,8 @@ struct XyArgs {
 };
 
 // K2 (SIGN = -1) / K4 (SIGN = +1): PB contiguous (x,y) planes per CTA.
-template <typename T, class SX, class SY, int SIGN, int PB, int NTHREADS>
-__global__ void __launch_bounds__(NTHREADS)
+template <typename T, class SX, class SY, int SIGN, int PB, int NTHREADS, int MINB>
+__global__ void __launch_bounds__(NTHREADS, MINB)
 fft_xy_ct(Cx<T>* __restrict__ D, const XyArgs A, const int* done) {
     extern __shared__ __align__(16) unsigned char smem_raw[];
     if (done && *reinterpret_cast<const volatile int*>(done)) return;
@@ -196,8 +196,8 @@ struct ZtArgs {
 };
 
 // K3: forward z, forward t, scale, inverse t, inverse z on CX contiguous (x,y)-plane sites.
-template <typename T, class SZ, class ST_, int CX, int NTHREADS>
-__global__ void __launch_bounds__(NTHREADS)
+template <typename T, class SZ, class ST_, int CX, int NTHREADS, int MINB>
+__global__ void __launch_bounds__(NTHREADS, MINB)
 fft_zt_ct(Cx<T>* __restrict__ D, const ZtArgs A, const int* done) {
     extern __shared__ __align__(16) unsigned char smem_raw[];
     if (done && *reinterpret_cast<const volatile int*>(done)) return;
