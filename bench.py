@@ -185,6 +185,7 @@ def main():
     import torch.distributed as dist
     import lgf_inputs as gi
     import paper_1208_1186_b200 as lgf
+    from paper_1208_1186_b200 import replicas
 
     world = int(os.environ.get("WORLD_SIZE", "1"))
     rank = int(os.environ.get("RANK", "0"))
@@ -201,7 +202,7 @@ def main():
     peak, peak_src = measured_peak()
 
     # every rank: its own seeded lattice (replicas only)
-    U = gi.make_config(L, gi.CONFIG_SEED + 2 + 1000 * rank, args.plaquette, device=dev)
+    U = gi.make_config(L, replicas.rank_seed(gi.CONFIG_SEED + 2, rank), args.plaquette, device=dev)
     plaq = gi.mean_plaquette(U, L)
 
     primary = (args.precision, args.storage)
@@ -238,10 +239,7 @@ def main():
         ms = e0.elapsed_time(e1)
         if sampler:
             clocks = sampler.stop()
-        if world > 1:
-            t = torch.tensor([ms], device=dev, dtype=torch.float64)
-            dist.all_reduce(t, op=dist.ReduceOp.MAX)
-            ms = float(t.item())
+        ms = replicas.max_over_ranks(ms, dev)
         kern_ms, _ = gf.profile_iterate(20, ALPHA)
         w = 8 if prec == "f64" else 4
         b_iter = (12 * stor + 64) * w
@@ -285,10 +283,7 @@ def main():
         gf.store(host_out)
         torch.cuda.synchronize()
         sec = time.perf_counter() - t0
-        if world > 1:
-            t = torch.tensor([sec], device=dev, dtype=torch.float64)
-            dist.all_reduce(t, op=dist.ReduceOp.MAX)
-            sec = float(t.item())
+        sec = replicas.max_over_ranks(sec, dev)
         nb = host_in.numel() * host_in.element_size()
         e2e = {"value": world * r.iterations / sec, "unit": "iterations/s",
                "h2d_bytes_per_step": nb / max(r.iterations, 1), "d2h_bytes_per_step": nb / max(r.iterations, 1),
