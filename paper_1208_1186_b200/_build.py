@@ -7,9 +7,9 @@ import subprocess
 _HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(_HERE, "csrc")
 LIB = os.path.join(_HERE, "liblgf.so")
-SOURCES = ["lgf_api.cu", "lgf_fft_inst.cu", "lgf_fft_inst_f64.cu", "lgf_fft_inst_f32.cu"]
+SOURCES = ["lgf_api.cu", "lgf_fft_inst.cu", "lgf_fft_inst_f64.cu", "lgf_fft_inst_f32.cu", "lgf_fft_pipe_f64.cu", "lgf_fft_pipe_f32.cu"]
 HEADERS = ["lgf_math.cuh", "lgf_site.cuh", "lgf_site_mu.cuh", "lgf_fft.cuh", "lgf_regfft.cuh", "lgf_fft_ct.cuh", "lgf_fft_inst.cuh",
-           "lgf_fft_inst_impl.cuh", os.path.join("..", "..", "include", "lgf.h")]
+           "lgf_fft_inst_impl.cuh", "lgf_async.cuh", "lgf_fft_pipe.cuh", "lgf_fft_pipe_inst.cuh", "lgf_fft_pipe_inst_impl.cuh", os.path.join("..", "..", "include", "lgf.h")]
 
 NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo", "-O3", "-std=c++17", "-Xcompiler", "-fPIC"]
 LINK_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-shared", "--cudart", "shared"]

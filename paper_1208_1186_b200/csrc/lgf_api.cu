@@ -14,6 +14,8 @@
 #include "lgf_fft.cuh"
 #include "lgf_fft_ct.cuh"
 #include "lgf_fft_inst.cuh"
+#include "lgf_fft_pipe.cuh"
+#include "lgf_fft_pipe_inst.cuh"
 #include "lgf_site.cuh"
 #include "lgf_site_mu.cuh"
 
@@ -70,7 +72,7 @@ bool factor23(int n, Axis* ax) {
 }
 
 struct Layout {          // byte offsets into the workspace
-    size_t state, partials, tw[4], twi[4], psq[4], links, delta, staging, total;
+    size_t state, partials, tw[4], twi[4], psq[4], links, delta, delta2, staging, total;
     int nblocks_site;
     int nb[4];
     int nblocks_mu;          // tiling of the (site, direction) kernels
@@ -108,6 +110,8 @@ Layout make_layout(const int32_t L[4], int precision, int storage) {
     for (int i = 0; i < 4; ++i) { lo.psq[i] = off; off += align_up((size_t)L[i] * w); }
     lo.links = off; off += align_up(4 * (size_t)(storage / 2) * V * 2 * w);
     lo.delta = off; off += align_up(4 * V * 2 * w);
+    // layout-B spectrum between K2 and K3 (pipelined FFT path): tiles padded by one z entry per t row
+    lo.delta2 = off; off += align_up(4 * (V / L[2]) * (size_t)(L[2] + 1) * 2 * w);
     const size_t stage_sites = V < (size_t)kStageSites ? V : (size_t)kStageSites;
     lo.staging = off; off += align_up(stage_sites * 36 * 2 * w);
     lo.total = off;
@@ -141,6 +145,11 @@ struct lgf_ctx {
     const ZtCtEntry* zt_ct;
     XyArgs xy_args;
     ZtArgs zt_args;
+    // pipelined fast path (lgf_fft_pipe.cuh); both set or both null
+    const XyPipeEntry* xy_pipe;
+    const ZtPipeEntry* zt_pipe;
+    XyPipeArgs xyp_args;
+    int xyp_grid, ztp_grid;
     bool loaded, delta_valid;
     int64_t launches;
     // iteration graph (K2 K3 K4 K5 K1), captured per alpha
@@ -237,13 +246,34 @@ bool plan_passes(lgf_ctx* c) {
     // spectrum in digit-swapped order, which only the compile-time K3 knows how to un-swap
     c->zt_ct = find_zt_ct(c->precision, L[2], L[3], LxLy);
     c->xy_ct = c->zt_ct ? find_xy_ct(c->precision, L[0], L[1]) : nullptr;
-    if (getenv("LGF_FORCE_GENERIC_FFT")) c->xy_ct = nullptr, c->zt_ct = nullptr;
+    c->zt_pipe = find_zt_pipe(c->precision, L[2], L[3], LxLy);
+    c->xy_pipe = c->zt_pipe ? find_xy_pipe(c->precision, L[0], L[1]) : nullptr;
+    if (!c->xy_pipe) c->zt_pipe = nullptr;
+    {   // LGF_FFT_PIPE=0: fall back to the one-tile-per-CTA kernels (A/B knob)
+        const char* e = getenv("LGF_FFT_PIPE");
+        if (e && atoi(e) == 0) c->xy_pipe = nullptr, c->zt_pipe = nullptr;
+    }
+    if (getenv("LGF_FORCE_GENERIC_FFT")) c->xy_ct = nullptr, c->zt_ct = nullptr, c->xy_pipe = nullptr, c->zt_pipe = nullptr;
     if (c->xy_ct) {
         c->xy_args.twx_fwd = c->axis[0].tw_fwd; c->xy_args.twx_inv = c->axis[0].tw_inv;
         c->xy_args.twy_fwd = c->axis[1].tw_fwd; c->xy_args.twy_inv = c->axis[1].tw_inv;
         c->xy_args.nplanes = (int)(4 * LzLt);
     }
-    if (c->zt_ct) {
+    if (c->xy_pipe) {
+        XyPipeArgs& P = c->xyp_args;
+        P.twx_fwd = c->axis[0].tw_fwd; P.twx_inv = c->axis[0].tw_inv;
+        P.twy_fwd = c->axis[1].tw_fwd; P.twy_inv = c->axis[1].tw_inv;
+        P.nplanes = (int)(4 * LzLt);
+        P.planes_per_comp = (int)LzLt;
+        P.nz = L[2];
+        P.pt = c->zt_pipe->cx * (L[2] + 1);
+        P.tile_elems = P.pt * L[3];
+        int sh = 0;
+        while ((1 << sh) < c->zt_pipe->cx) ++sh;
+        P.cxb_shift = sh;
+        P.chunks_per_comp = (int)(LxLy >> sh);
+    }
+    if (c->zt_ct || c->zt_pipe) {
         ZtArgs& A = c->zt_args;
         A.twz_fwd = c->axis[2].tw_fwd; A.twz_inv = c->axis[2].tw_inv;
         A.twt_fwd = c->axis[3].tw_fwd; A.twt_inv = c->axis[3].tw_inv;
@@ -251,11 +281,11 @@ bool plan_passes(lgf_ctx* c) {
         A.V = c->V;
         A.LxLy = LxLy;
         A.Lx = L[0];
-        A.tiles_per_comp = (int)(LxLy / c->zt_ct->cx);
+        A.tiles_per_comp = (int)(LxLy / (c->zt_pipe ? c->zt_pipe->cx : c->zt_ct->cx));
         A.scale_num = Z.scale_num;
-        A.x_n1 = c->xy_ct ? c->xy_ct->x_n1 : L[0];
+        A.x_n1 = c->xy_pipe ? c->xy_pipe->x_n1 : (c->xy_ct ? c->xy_ct->x_n1 : L[0]);
         A.x_n2 = L[0] / A.x_n1;
-        A.y_n1 = c->xy_ct ? c->xy_ct->y_n1 : L[1];
+        A.y_n1 = c->xy_pipe ? c->xy_pipe->y_n1 : (c->xy_ct ? c->xy_ct->y_n1 : L[1]);
         A.y_n2 = L[1] / A.y_n1;
     }
     return true;
@@ -340,6 +370,21 @@ struct Impl {
         const int* done = gated ? &dev_state(c)->done : nullptr;
         const unsigned planes = (unsigned)(4 * (long long)c->L[2] * c->L[3]);
         Cx<T>* dptr = delta(c);
+        if (c->xy_pipe) {
+            Cx<T>* d2 = reinterpret_cast<Cx<T>*>(c->ws + c->lo.delta2);
+            if (k == 1) {
+                const ZtPipeEntry* e = c->zt_pipe;
+                void* args[] = {&d2, &dptr, &c->zt_args, &done};          // layout B -> natural
+                CU(cudaLaunchKernel(e->kernel, dim3(c->ztp_grid), dim3(e->threads), args, e->smem, c->stream));
+            } else {
+                const XyPipeEntry* e = c->xy_pipe;
+                Cx<T>* outp = k == 0 ? d2 : dptr;                          // K2: natural -> layout B; K4: in place
+                void* args[] = {&dptr, &outp, &c->xyp_args, &done};
+                CU(cudaLaunchKernel(k == 0 ? e->k_fwd : e->k_inv, dim3(c->xyp_grid), dim3(e->threads), args, e->smem, c->stream));
+            }
+            c->launches++;
+            return LGF_OK;
+        }
         if (k != 1 && c->xy_ct) {
             const XyCtEntry* e = c->xy_ct;
             void* args[] = {&dptr, &c->xy_args, &done};
@@ -369,6 +414,20 @@ struct Impl {
         CU(cudaFuncSetAttribute(fft_xy_kernel<T, +1>, cudaFuncAttributeMaxDynamicSharedMemorySize, kMaxSmem));
         CU(cudaFuncSetAttribute(fft_zt_kernel<T>, cudaFuncAttributeMaxDynamicSharedMemorySize, kMaxSmem));
         CU(prepare_ct_kernels(c->precision));
+        CU(prepare_pipe_kernels(c->precision));
+        if (c->xy_pipe) {   // persistent grids: one CTA per SM (or fewer when there are fewer tiles)
+            int dev = 0, sms = 0, occ = 0;
+            CU(cudaGetDevice(&dev));
+            CU(cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev));
+            const int xy_tiles = (c->xyp_args.nplanes + c->xy_pipe->pb - 1) / c->xy_pipe->pb;
+            CU(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, c->xy_pipe->k_fwd, c->xy_pipe->threads, c->xy_pipe->smem));
+            if (occ < 1) return cuda_fail(cudaErrorLaunchOutOfResources, "fft_xy_pipe does not fit on an SM");
+            c->xyp_grid = xy_tiles < occ * sms ? xy_tiles : occ * sms;
+            const int zt_tiles = 4 * c->zt_args.tiles_per_comp;
+            CU(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, c->zt_pipe->kernel, c->zt_pipe->threads, c->zt_pipe->smem));
+            if (occ < 1) return cuda_fail(cudaErrorLaunchOutOfResources, "fft_zt_pipe does not fit on an SM");
+            c->ztp_grid = zt_tiles < occ * sms ? zt_tiles : occ * sms;
+        }
         return upload_tables<T>(c);
     }
     static int load(lgf_ctx* c, const void* src, int memspace) {

@@ -26,20 +26,24 @@ template <int N, int N1> struct LineSplit {
 
 // ---- the four stage bodies; LD(pos) / ST(pos, value) address one line, pos in [0, N) ----------
 // tw: table exp(-2 pi i j / N) (forward) or exp(+2 pi i j / N) (inverse), j < N, in global memory.
-template <typename T, class S, class LD, class ST>
+// WSYNC = 1: a warp-level barrier between the loads and the stores, for callers whose store addresses
+// are another lane's load addresses (the swizzling first stage of lgf_fft_pipe.cuh).
+template <typename T, class S, int WSYNC = 0, class LD, class ST>
 __device__ __forceinline__ void stage_A_fwd(int n2, const Cx<T>* __restrict__ tw, LD&& ld, ST&& st) {
     Cx<T> v[S::kN1];
     static_for<0, S::kN1>([&](auto m) { v[m.value] = ld(n2 + S::kN2 * m.value); });
+    if constexpr (WSYNC) __syncwarp();
     RegFft<S::kN1, -1, T>::run(v);
     if constexpr (S::kN2 > 1) {
         static_for<1, S::kN1>([&](auto k1) { v[k1.value] = v[k1.value] * ldg_cx(tw + n2 * k1.value); });
     }
     static_for<0, S::kN1>([&](auto k1) { st(k1.value * S::kN2 + n2, v[k1.value]); });
 }
-template <typename T, class S, class LD, class ST>
+template <typename T, class S, int WSYNC = 0, class LD, class ST>
 __device__ __forceinline__ void stage_A_inv(int n2, LD&& ld, ST&& st) {
     Cx<T> v[S::kN1];
     static_for<0, S::kN1>([&](auto k1) { v[k1.value] = ld(k1.value * S::kN2 + n2); });
+    if constexpr (WSYNC) __syncwarp();
     RegFft<S::kN1, +1, T>::run(v);
     static_for<0, S::kN1>([&](auto m) { st(n2 + S::kN2 * m.value, v[m.value]); });
 }
@@ -47,10 +51,11 @@ struct NoScale {};
 
 // B forward, optional scale (SC(k2) -> multiplier for frequency k1 + N1 k2), B' inverse: all on the
 // same thread <-> element mapping, so they chain in registers.
-template <typename T, class S, int DO_FWD, int DO_INV, class LD, class ST, class SC>
+template <typename T, class S, int DO_FWD, int DO_INV, int WSYNC = 0, class LD, class ST, class SC>
 __device__ __forceinline__ void stage_B(int k1, const Cx<T>* __restrict__ tw_inv, LD&& ld, ST&& st, SC&& sc) {
     Cx<T> v[S::kN2];
     static_for<0, S::kN2>([&](auto j) { v[j.value] = ld(k1 * S::kN2 + j.value); });
+    if constexpr (WSYNC) __syncwarp();
     if constexpr (DO_FWD) {
         RegFft<S::kN2, -1, T>::run(v);
         if constexpr (!std::is_same<typename std::decay<SC>::type, NoScale>::value) {

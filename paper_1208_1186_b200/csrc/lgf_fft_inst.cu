@@ -1,5 +1,6 @@
 // lgf_fft_inst.cu -- lookup over the instantiation tables of the compile-time-sized FFT kernels.
 #include "lgf_fft_inst.cuh"
+#include "lgf_fft_pipe_inst.cuh"
 
 #include <cstdlib>
 
@@ -49,6 +50,49 @@ cudaError_t prepare_ct_kernels(int precision) {
     const ZtCtEntry* z = zt_tab(precision, &n);
     for (int i = 0; i < n; ++i) {
         if (z[i].smem <= 48 * 1024) continue;
+        cudaError_t e = cudaFuncSetAttribute(z[i].kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)z[i].smem);
+        if (e != cudaSuccess) return e;
+    }
+    return cudaSuccess;
+}
+
+
+// ---- pipelined kernels (lgf_fft_pipe.cuh) ----
+static const XyPipeEntry* xyp_tab(int precision, int* n) { return precision ? xy_pipe_table_f64(n) : xy_pipe_table_f32(n); }
+static const ZtPipeEntry* ztp_tab(int precision, int* n) { return precision ? zt_pipe_table_f64(n) : zt_pipe_table_f32(n); }
+
+const XyPipeEntry* find_xy_pipe(int precision, int nx, int ny) {
+    int n = 0, skip = variant("LGF_XYP_VARIANT");
+    const XyPipeEntry* t = xyp_tab(precision, &n);
+    const XyPipeEntry* last = nullptr;
+    for (int i = 0; i < n; ++i)
+        if (t[i].nx == nx && t[i].ny == ny) {
+            last = &t[i];
+            if (skip-- == 0) return last;
+        }
+    return last;
+}
+const ZtPipeEntry* find_zt_pipe(int precision, int nz, int nt, long long LxLy) {
+    int n = 0, skip = variant("LGF_ZTP_VARIANT");
+    const ZtPipeEntry* t = ztp_tab(precision, &n);
+    const ZtPipeEntry* last = nullptr;
+    for (int i = 0; i < n; ++i)
+        if (t[i].nz == nz && t[i].nt == nt && LxLy % t[i].cx == 0) {
+            last = &t[i];
+            if (skip-- == 0) return last;
+        }
+    return last;
+}
+cudaError_t prepare_pipe_kernels(int precision) {
+    int n = 0;
+    const XyPipeEntry* x = xyp_tab(precision, &n);
+    for (int i = 0; i < n; ++i) {
+        cudaError_t e = cudaFuncSetAttribute(x[i].k_fwd, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)x[i].smem);
+        if (e == cudaSuccess) e = cudaFuncSetAttribute(x[i].k_inv, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)x[i].smem);
+        if (e != cudaSuccess) return e;
+    }
+    const ZtPipeEntry* z = ztp_tab(precision, &n);
+    for (int i = 0; i < n; ++i) {
         cudaError_t e = cudaFuncSetAttribute(z[i].kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)z[i].smem);
         if (e != cudaSuccess) return e;
     }

@@ -1,0 +1,33 @@
+// fp64 instantiations of the pipelined FFT kernels.  <T, N, N1, M, M1, PB|CX, GT, NG, NBUF>:
+// N1 = N means "whole line in registers"; 48 = 8*6 and 64 = 8*8 take two register stages.
+#include "lgf_fft_pipe_inst_impl.cuh"
+
+namespace lgf {
+using namespace pinst;
+typedef double T;
+
+const XyPipeEntry* xy_pipe_table_f64(int* n) {
+    static const XyPipeEntry tab[] = {
+        XyP<T, 8, 8, 8, 8, 16, 128, 2, 3>::entry(),
+        XyP<T, 16, 16, 16, 16, 8, 128, 2, 3>::entry(),
+        XyP<T, 32, 32, 32, 32, 4, 128, 2, 3>::entry(),
+        XyP<T, 32, 32, 32, 32, 2, 64, 4, 6>::entry(),
+        XyP<T, 48, 8, 48, 8, 1, 256, 2, 4>::entry(),
+        XyP<T, 64, 8, 64, 8, 1, 256, 2, 3>::entry(),
+    };
+    *n = (int)(sizeof(tab) / sizeof(tab[0]));
+    return tab;
+}
+const ZtPipeEntry* zt_pipe_table_f64(int* n) {
+    static const ZtPipeEntry tab[] = {
+        ZtP<T, 8, 8, 8, 8, 8, 64, 2, 3>::entry(),
+        ZtP<T, 16, 16, 16, 16, 4, 64, 2, 3>::entry(),
+        ZtP<T, 32, 32, 32, 32, 4, 128, 2, 3>::entry(),
+        ZtP<T, 32, 32, 32, 32, 2, 64, 4, 6>::entry(),
+        ZtP<T, 48, 8, 8, 8, 8, 256, 2, 4>::entry(),
+        ZtP<T, 64, 8, 64, 8, 2, 512, 1, 1>::entry(),
+    };
+    *n = (int)(sizeof(tab) / sizeof(tab[0]));
+    return tab;
+}
+}  // namespace lgf

@@ -1,0 +1,40 @@
+// lgf_fft_pipe_inst.cuh -- registry of the pipelined FFT kernels (lgf_fft_pipe.cuh).
+// lgf_fft_pipe_f64.cu / lgf_fft_pipe_f32.cu instantiate the tables; lgf_api.cu looks kernels up by
+// lattice extents.  A lattice runs on this path when BOTH its (x,y) and its (z,t) extents are
+// instantiated (K2 writes layout B for exactly the chunk size K3 was compiled for).
+#pragma once
+#include <cuda_runtime.h>
+#include <stddef.h>
+
+namespace lgf {
+
+struct XyPipeEntry {
+    int nx, ny;
+    int x_n1, y_n1;          // first-stage radices (digit-swapped spectrum order, see lgf_fft_ct.cuh)
+    int pb;                  // planes per tile
+    int threads;             // GT * NG
+    int nbuf;
+    size_t smem;
+    const void* k_fwd;       // fft_xy_pipe<..., -1, ...>  natural -> layout B
+    const void* k_inv;       // fft_xy_pipe<..., +1, ...>  natural -> natural
+};
+struct ZtPipeEntry {
+    int nz, nt;
+    int cx;                  // tile width = layout-B chunk (power of two, divides Lx*Ly)
+    int threads;
+    int nbuf;
+    size_t smem;
+    const void* kernel;      // fft_zt_pipe<...>  layout B -> natural
+};
+
+// precision: 0 = float, 1 = double; LGF_XYP_VARIANT / LGF_ZTP_VARIANT pick the v-th match (A/B knob)
+const XyPipeEntry* find_xy_pipe(int precision, int nx, int ny);
+const ZtPipeEntry* find_zt_pipe(int precision, int nz, int nt, long long LxLy);
+cudaError_t prepare_pipe_kernels(int precision);
+
+const XyPipeEntry* xy_pipe_table_f64(int* n);
+const ZtPipeEntry* zt_pipe_table_f64(int* n);
+const XyPipeEntry* xy_pipe_table_f32(int* n);
+const ZtPipeEntry* zt_pipe_table_f32(int* n);
+
+}  // namespace lgf

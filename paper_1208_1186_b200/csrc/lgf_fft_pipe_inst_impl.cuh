@@ -1,0 +1,35 @@
+// lgf_fft_pipe_inst_impl.cuh -- entry builders shared by the two instantiation units.
+#pragma once
+#include "lgf_fft_pipe.cuh"
+#include "lgf_fft_pipe_inst.cuh"
+
+namespace lgf {
+namespace pinst {
+
+template <typename T, int NX, int X1, int NY, int Y1, int PB, int GT, int NG, int NBUF>
+struct XyP {
+    typedef LineSplit<NX, X1> SX;
+    typedef LineSplit<NY, Y1> SY;
+    static constexpr size_t kSmem = sizeof(Cx<T>) * (size_t)NBUF * PB * NX * NY + 8 * NBUF;
+    static_assert(kSmem <= 227 * 1024, "tile ring exceeds shared memory");
+    static XyPipeEntry entry() {
+        return XyPipeEntry{NX, NY, X1, Y1, PB, GT * NG, NBUF, kSmem,
+                           (const void*)&fft_xy_pipe<T, SX, SY, -1, PB, GT, NG, NBUF>,
+                           (const void*)&fft_xy_pipe<T, SX, SY, +1, PB, GT, NG, NBUF>};
+    }
+};
+
+template <typename T, int NZ, int Z1, int NT, int T1, int CX, int GT, int NG, int NBUF>
+struct ZtP {
+    typedef LineSplit<NZ, Z1> SZ;
+    typedef LineSplit<NT, T1> ST_;
+    static constexpr size_t kSmem = sizeof(Cx<T>) * (size_t)NBUF * CX * (NZ + 1) * NT + 8 * NBUF;
+    static_assert(kSmem <= 227 * 1024, "tile ring exceeds shared memory");
+    static_assert((CX & (CX - 1)) == 0, "CX must be a power of two");
+    static ZtPipeEntry entry() {
+        return ZtPipeEntry{NZ, NT, CX, GT * NG, NBUF, kSmem, (const void*)&fft_zt_pipe<T, SZ, ST_, CX, GT, NG, NBUF>};
+    }
+};
+
+}  // namespace pinst
+}  // namespace lgf
