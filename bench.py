@@ -50,6 +50,8 @@ def parse_args():
 
 def bytes_per_site(kernel: str, n_l: int, w: int) -> int:
     """Algorithmic bytes per site."""
+    if kernel.startswith("K51"):
+        return (8 * n_l + 16) * w      # fused update: links read + written once, Delta~ read, Delta written
     if kernel.startswith("K1"):
         return (4 * n_l + 8) * w
     if kernel.startswith("K5"):

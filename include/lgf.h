@@ -122,6 +122,12 @@ int lgf_debug_fourier_accelerate(lgf_ctx* ctx);
  * K4 fft_xy_inv, K5 gbuild_update, K1 delta_theta_F.  For roofline reporting. */
 int lgf_profile_iterate(lgf_ctx* ctx, int64_t n, double alpha, double ms[5], lgf_result* out);
 
+/* Which kernels this context's iteration runs (for reports): info[0] = FFT path (0 runtime-radix,
+ * 1 compile-time-sized one-tile-per-CTA, 2 pipelined persistent), info[1] = 1 if K5 and K1 are fused
+ * into the marching update kernel (then ms[3] of lgf_profile_iterate is the fused kernel and ms[4] ~ 0),
+ * info[2] = CTAs of the site kernel, info[3] = kernel launches per iteration (0 before the first run). */
+int lgf_path_info(const lgf_ctx* ctx, int32_t info[4]);
+
 /* Number of kernel launches this context has enqueued since creation (for bench.py's gpu_launches). */
 int64_t lgf_launch_count(const lgf_ctx* ctx);
 

@@ -72,6 +72,7 @@ def load_library() -> ctypes.CDLL:
     lib.lgf_profile_iterate.argtypes = [vp, ctypes.c_int64, ctypes.c_double, ctypes.POINTER(ctypes.c_double), rp]
     lib.lgf_debug_get_delta.argtypes = [vp, vp, ctypes.c_int]
     lib.lgf_debug_fourier_accelerate.argtypes = [vp]
+    lib.lgf_path_info.argtypes = [vp, i32p]
     lib.lgf_launch_count.restype = ctypes.c_int64
     lib.lgf_launch_count.argtypes = [vp]
     for f in (lib.lgf_strerror, lib.lgf_last_error, lib.lgf_version):
@@ -187,14 +188,24 @@ class GaugeFixer:
         return self._res(r)
 
     KERNELS = ("K2_fft_xy_fwd", "K3_fft_zt_fwd_scale_inv", "K4_fft_xy_inv", "K5_gbuild_update", "K1_delta_theta_F")
+    KERNELS_FUSED = ("K2_fft_xy_fwd", "K3_fft_zt_fwd_scale_inv", "K4_fft_xy_inv", "K51_update_delta_fused")
+
+    def path_info(self) -> dict:
+        """Which kernels the iteration runs: fft_path 0/1/2, fused K5+K1, site-kernel CTAs, launches per iteration."""
+        info = (ctypes.c_int32 * 4)()
+        _check(self.lib.lgf_path_info(self._h, info), "lgf_path_info")
+        return {"fft_path": ("runtime-radix", "compile-time", "pipelined")[info[0]], "fused": bool(info[1]),
+                "site_ctas": int(info[2]), "launches_per_iteration": int(info[3])}
 
     def profile_iterate(self, n: int, alpha: float):
-        """-> (dict kernel name -> average ms per launch, LgfResult)."""
+        """-> (dict kernel name -> average ms per launch, LgfResult).  With the fused update kernel the
+        dict has four entries (K5 and K1 are one kernel)."""
         ms = (ctypes.c_double * 5)()
         r = _Result()
         with self._torch.cuda.device(self.device):
             _check(self.lib.lgf_profile_iterate(self._h, int(n), float(alpha), ms, ctypes.byref(r)), "lgf_profile_iterate")
-        return {k: float(ms[i]) for i, k in enumerate(self.KERNELS)}, self._res(r)
+        names = self.KERNELS_FUSED if self.path_info()["fused"] else self.KERNELS
+        return {k: float(ms[i]) for i, k in enumerate(names)}, self._res(r)
 
     def debug_delta(self):
         """Packed Delta field as a host tensor [V,4,2]."""

@@ -18,6 +18,7 @@
 #include "lgf_fft_pipe_inst.cuh"
 #include "lgf_site.cuh"
 #include "lgf_site_mu.cuh"
+#include "lgf_site_fused.cuh"
 
 using namespace lgf;
 
@@ -72,7 +73,7 @@ bool factor23(int n, Axis* ax) {
 }
 
 struct Layout {          // byte offsets into the workspace
-    size_t state, partials, tw[4], twi[4], psq[4], links, delta, delta2, staging, total;
+    size_t state, partials, tw[4], twi[4], psq[4], links, links_bytes, delta, delta2, delta3, staging, total;
     int nblocks_site;
     int nb[4];
     int nblocks_mu;          // tiling of the (site, direction) kernels
@@ -108,10 +109,13 @@ Layout make_layout(const int32_t L[4], int precision, int storage) {
     for (int i = 0; i < 4; ++i) { lo.tw[i] = off; off += align_up((size_t)L[i] * 2 * w); }
     for (int i = 0; i < 4; ++i) { lo.twi[i] = off; off += align_up((size_t)L[i] * 2 * w); }
     for (int i = 0; i < 4; ++i) { lo.psq[i] = off; off += align_up((size_t)L[i] * w); }
-    lo.links = off; off += align_up(4 * (size_t)(storage / 2) * V * 2 * w);
+    // two link buffers: the fused update kernel writes the new field out of place (DevState::cur)
+    lo.links_bytes = align_up(4 * (size_t)(storage / 2) * V * 2 * w);
+    lo.links = off; off += 2 * lo.links_bytes;
     lo.delta = off; off += align_up(4 * V * 2 * w);
     // layout-B spectrum between K2 and K3 (pipelined FFT path): tiles padded by one z entry per t row
     lo.delta2 = off; off += align_up(4 * (V / L[2]) * (size_t)(L[2] + 1) * 2 * w);
+    lo.delta3 = off; off += align_up(4 * V * 2 * w);   // Delta of the new links (fused path: K1/K51 out, K2 in)
     const size_t stage_sites = V < (size_t)kStageSites ? V : (size_t)kStageSites;
     lo.staging = off; off += align_up(stage_sites * 36 * 2 * w);
     lo.total = off;
@@ -150,6 +154,12 @@ struct lgf_ctx {
     const ZtPipeEntry* zt_pipe;
     XyPipeArgs xyp_args;
     int xyp_grid, ztp_grid;
+    // fused K5+K1 marching kernel (lgf_site_fused.cuh); -1: not used
+    int fused_tile;
+    MarchGeom mgeom;
+    int fused_grid;
+    int cur_host;                // host mirror of DevState::cur
+    bool dbg_delta_tilde;        // lgf_debug_get_delta source: Delta~ (after debug_fourier_accelerate) or Delta
     bool loaded, delta_valid;
     int64_t launches;
     // iteration graph (K2 K3 K4 K5 K1), captured per alpha
@@ -166,6 +176,7 @@ namespace {
 
 DevState* dev_state(lgf_ctx* c) { return reinterpret_cast<DevState*>(c->ws + c->lo.state); }
 
+__global__ void reset_cur_kernel(DevState* st) { st->cur = 0; }
 __global__ void init_state_kernel(DevState* st, double tol, long long max_iter) {
     st->iter = 0;
     st->done = 0;
@@ -316,8 +327,11 @@ int upload_tables(lgf_ctx* c) {
 // ---- typed launchers ---------------------------------------------------------------------------
 template <typename T, int NC>
 struct Impl {
-    static Cx<T>* links(lgf_ctx* c) { return reinterpret_cast<Cx<T>*>(c->ws + c->lo.links); }
-    static Cx<T>* delta(lgf_ctx* c) { return reinterpret_cast<Cx<T>*>(c->ws + c->lo.delta); }
+    static Cx<T>* links_buf(lgf_ctx* c, int which) { return reinterpret_cast<Cx<T>*>(c->ws + c->lo.links + (size_t)which * c->lo.links_bytes); }
+    static Cx<T>* links(lgf_ctx* c) { return links_buf(c, c->cur_host); }     // the current field, as the host knows it
+    static Cx<T>* delta(lgf_ctx* c) { return reinterpret_cast<Cx<T>*>(c->ws + c->lo.delta); }      // Delta~ (natural)
+    // where K1 / K51 write Delta of the current links and K2 reads it
+    static Cx<T>* delta_src(lgf_ctx* c) { return reinterpret_cast<Cx<T>*>(c->ws + (c->fused_tile >= 0 ? c->lo.delta3 : c->lo.delta)); }
     static Cx<T>* staging(lgf_ctx* c) { return reinterpret_cast<Cx<T>*>(c->ws + c->lo.staging); }
 
     static int k1(lgf_ctx* c, int mode) {
@@ -326,11 +340,11 @@ struct Impl {
         {
             nblocks = c->lo.nblocks_site;
 #define LGF_K1_CASE(ID, TILE) case ID: k1_delta_theta_F<T, NC, TILE><<<nblocks, TILE::kThreads, 0, c->stream>>>( \
-                links(c), delta(c), partials, dev_state(c), c->geom, mode); break;
+                links(c), delta_src(c), partials, dev_state(c), c->geom, mode); break;
             switch (c->site_tile) {
                 LGF_K1_CASE(1, Tile1) LGF_K1_CASE(2, Tile2) LGF_K1_CASE(3, Tile3) LGF_K1_CASE(4, Tile4) LGF_K1_CASE(5, Tile5)
                 default: k1_delta_theta_F<T, NC, Tile0><<<nblocks, Tile0::kThreads, 0, c->stream>>>(
-                    links(c), delta(c), partials, dev_state(c), c->geom, mode);
+                    links(c), delta_src(c), partials, dev_state(c), c->geom, mode);
             }
 #undef LGF_K1_CASE
         }
@@ -338,6 +352,75 @@ struct Impl {
         k1_finish<<<1, 256, 0, c->stream>>>(partials, nblocks, dev_state(c), (double)c->V, mode);
         c->launches += 2;
         CU(cudaGetLastError());
+        return LGF_OK;
+    }
+    // fused K5 + K1: update out of place, emit Delta/theta/F of the new links, swap the link buffers
+    static int k51(lgf_ctx* c, double alpha) {
+        double2* partials = reinterpret_cast<double2*>(c->ws + c->lo.partials);
+        const Cx<T>* u0 = links_buf(c, 0);
+        const Cx<T>* u1 = links_buf(c, 1);
+        const Cx<T>* dt = delta(c);
+        Cx<T>* dout = delta_src(c);
+        const DevState* st = dev_state(c);
+        T ha = (T)(0.5 * alpha);
+        void* args[] = {&u0, &u1, &dt, &dout, &partials, &st, &c->mgeom, &ha};
+        const FusedEntry& e = fused_entries()[c->fused_tile];
+        CU(cudaLaunchKernel(e.kernel, dim3(c->fused_grid), dim3(e.threads), args, e.smem, c->stream));
+        k1_finish<<<1, 256, 0, c->stream>>>(partials, c->fused_grid, dev_state(c), (double)c->V, 2);
+        c->launches += 2;
+        CU(cudaGetLastError());
+        return LGF_OK;
+    }
+    struct FusedEntry { int tx, ty, tz, threads; size_t smem; const void* kernel; };
+    template <class Tile, int MINB> static FusedEntry fused_entry() {
+        return FusedEntry{Tile::TX, Tile::TY, Tile::TZ, Tile::NS, Tile::template smem_bytes<T>(),
+                          (const void*)&k51_update_delta<T, NC, Tile, MINB>};
+    }
+    static const FusedEntry* fused_entries() {
+        static const FusedEntry tab[] = {
+            fused_entry<MarchTile<32, 4, 2>, 2>(),
+            fused_entry<MarchTile<64, 2, 2>, 2>(),
+            fused_entry<MarchTile<48, 4, 1>, 2>(),
+            fused_entry<MarchTile<16, 4, 4>, 2>(),
+            fused_entry<MarchTile<8, 8, 4>, 2>(),
+            fused_entry<MarchTile<32, 4, 4>, 1>(),
+            fused_entry<MarchTile<48, 4, 2>, 1>(),
+            fused_entry<MarchTile<64, 4, 2>, 1>(),
+        };
+        return tab;
+    }
+    static constexpr int kNumFused = 8;
+    // pick the marching tile for this lattice (LGF_FUSED = 0 disables the fused path, LGF_FUSED_TILE = i forces entry i)
+    static int plan_fused(lgf_ctx* c) {
+        c->fused_tile = -1;
+        if (!c->xy_pipe) return LGF_OK;                    // the fused path rides on the pipelined FFT buffers
+        const char* e = getenv("LGF_FUSED");
+        if (!e || atoi(e) == 0) return LGF_OK;             // opt-in (LGF_FUSED=1) until it beats K5 + K1 everywhere
+        const char* ft = getenv("LGF_FUSED_TILE");
+        const FusedEntry* tab = fused_entries();
+        for (int i = 0; i < kNumFused; ++i) {
+            if (ft && atoi(ft) != i) continue;
+            if (tab[i].tx != c->L[0] || c->L[1] % tab[i].ty || c->L[2] % tab[i].tz) continue;
+            c->fused_tile = i;
+            break;
+        }
+        if (c->fused_tile < 0) return LGF_OK;
+        const FusedEntry& fe = tab[c->fused_tile];
+        CU(cudaFuncSetAttribute(fe.kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)fe.smem));
+        int dev = 0, sms = 0, occ = 0;
+        CU(cudaGetDevice(&dev));
+        CU(cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev));
+        CU(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, fe.kernel, fe.threads, fe.smem));
+        if (occ < 1) { c->fused_tile = -1; return LGF_OK; }
+        MarchGeom& m = c->mgeom;
+        for (int i = 0; i < 4; ++i) m.L[i] = c->L[i];
+        m.V = c->V;
+        m.nby = c->L[1] / fe.ty;
+        m.nbz = c->L[2] / fe.tz;
+        m.nslices = (long long)m.nby * m.nbz * c->L[3];
+        long long grid = (long long)occ * sms;
+        if (grid > m.nslices) grid = m.nslices;
+        c->fused_grid = (int)grid;
         return LGF_OK;
     }
     static int k5(lgf_ctx* c, double alpha) {
@@ -378,8 +461,9 @@ struct Impl {
                 CU(cudaLaunchKernel(e->kernel, dim3(c->ztp_grid), dim3(e->threads), args, e->smem, c->stream));
             } else {
                 const XyPipeEntry* e = c->xy_pipe;
+                Cx<T>* inp = k == 0 ? delta_src(c) : dptr;                 // K2 reads Delta where K1 / K51 left it
                 Cx<T>* outp = k == 0 ? d2 : dptr;                          // K2: natural -> layout B; K4: in place
-                void* args[] = {&dptr, &outp, &c->xyp_args, &done};
+                void* args[] = {&inp, &outp, &c->xyp_args, &done};
                 CU(cudaLaunchKernel(k == 0 ? e->k_fwd : e->k_inv, dim3(c->xyp_grid), dim3(e->threads), args, e->smem, c->stream));
             }
             c->launches++;
@@ -428,11 +512,19 @@ struct Impl {
             if (occ < 1) return cuda_fail(cudaErrorLaunchOutOfResources, "fft_zt_pipe does not fit on an SM");
             c->ztp_grid = zt_tiles < occ * sms ? zt_tiles : occ * sms;
         }
+        {
+            const int rc = plan_fused(c);
+            if (rc) return rc;
+        }
         return upload_tables<T>(c);
     }
     static int load(lgf_ctx* c, const void* src, int memspace) {
         const long long V = c->V;
         const int thr = 256;
+        c->cur_host = 0;                                   // a fresh field always lands in buffer 0
+        reset_cur_kernel<<<1, 1, 0, c->stream>>>(dev_state(c));
+        c->launches++;
+        CU(cudaGetLastError());
         if (memspace == LGF_DEVICE) {
             const long long n = V * 36;
             aos_to_soa<T, NC><<<(unsigned)((n + thr - 1) / thr), thr, 0, c->stream>>>(
@@ -481,8 +573,9 @@ struct Impl {
     static int get_delta(lgf_ctx* c, void* dst, int memspace) {
         const long long V = c->V;
         const int thr = 256;
+        Cx<T>* srcp = c->dbg_delta_tilde ? delta(c) : delta_src(c);
         if (memspace == LGF_DEVICE) {
-            delta_to_aos<T><<<(unsigned)((V * 4 + thr - 1) / thr), thr, 0, c->stream>>>(delta(c), reinterpret_cast<Cx<T>*>(dst), V);
+            delta_to_aos<T><<<(unsigned)((V * 4 + thr - 1) / thr), thr, 0, c->stream>>>(srcp, reinterpret_cast<Cx<T>*>(dst), V);
             c->launches++;
             CU(cudaGetLastError());
             CU(cudaStreamSynchronize(c->stream));
@@ -490,7 +583,7 @@ struct Impl {
         }
         // host: copy the four component planes and interleave on the host side of the copy
         std::vector<Cx<T>> tmp((size_t)4 * V);
-        CU(cudaMemcpyAsync(tmp.data(), delta(c), (size_t)4 * V * sizeof(Cx<T>), cudaMemcpyDeviceToHost, c->stream));
+        CU(cudaMemcpyAsync(tmp.data(), srcp, (size_t)4 * V * sizeof(Cx<T>), cudaMemcpyDeviceToHost, c->stream));
         CU(cudaStreamSynchronize(c->stream));
         Cx<T>* out = reinterpret_cast<Cx<T>*>(dst);
         for (long long s = 0; s < V; ++s)
@@ -509,6 +602,7 @@ int enqueue_iteration_body(lgf_ctx* c, double alpha) {
     if ((rc = DISPATCH(c, fft(c, 0, true)))) return rc;
     if ((rc = DISPATCH(c, fft(c, 1, true)))) return rc;
     if ((rc = DISPATCH(c, fft(c, 2, true)))) return rc;
+    if (c->fused_tile >= 0) return DISPATCH(c, k51(c, alpha));
     if ((rc = DISPATCH(c, k5(c, alpha)))) return rc;
     if ((rc = DISPATCH(c, k1(c, 1)))) return rc;
     return LGF_OK;
@@ -706,6 +800,7 @@ static int finish(lgf_ctx* c, lgf_result* out, bool fix_mode) {
     if (rc) return rc;
     CU(cudaStreamSynchronize(c->stream));
     const DevState& s = c->host_state[0];
+    c->cur_host = s.cur;
     if (out) {
         out->iterations = s.iter;
         out->theta = s.theta;
@@ -722,6 +817,7 @@ int lgf_measure(lgf_ctx* c, lgf_result* out) {
     if (!rc) rc = DISPATCH(c, k1(c, 0));
     if (rc) return rc;
     c->delta_valid = true;
+    c->dbg_delta_tilde = false;
     lgf_result r;
     rc = finish(c, &r, false);
     if (rc) return rc;
@@ -736,7 +832,7 @@ int lgf_iterate_async(lgf_ctx* c, int64_t n, double alpha) {
     int rc = ensure_graph(c, alpha);
     if (!rc) rc = init_state(c, -1.0, (long long)n);
     if (!rc && (!c->delta_valid || n == 0)) rc = DISPATCH(c, k1(c, 0));
-    if (!rc) { c->delta_valid = true; rc = enqueue_iterations(c, n); }
+    if (!rc) { c->delta_valid = true; c->dbg_delta_tilde = false; rc = enqueue_iterations(c, n); }
     if (rc) return rc;
     c->pending_n = n;
     return LGF_OK;
@@ -768,6 +864,7 @@ int lgf_fix(lgf_ctx* c, double alpha, double theta_tol, int64_t max_iter, lgf_re
     if (!rc) rc = DISPATCH(c, k1(c, 0));
     if (rc) return rc;
     c->delta_valid = true;
+    c->dbg_delta_tilde = false;
     initial_test_kernel<<<1, 1, 0, c->stream>>>(dev_state(c));
     c->launches++;
     CU(cudaGetLastError());
@@ -816,6 +913,7 @@ int lgf_debug_fourier_accelerate(lgf_ctx* c) {
     for (int k = 0; k < 3; ++k)
         if ((rc = DISPATCH(c, fft(c, k, false)))) return rc;
     c->delta_valid = false;
+    c->dbg_delta_tilde = true;
     CU(cudaStreamSynchronize(c->stream));
     return LGF_OK;
 }
@@ -827,6 +925,7 @@ int lgf_profile_iterate(lgf_ctx* c, int64_t n, double alpha, double ms[5], lgf_r
     if (!rc && !c->delta_valid) rc = DISPATCH(c, k1(c, 0));
     if (rc) return rc;
     c->delta_valid = true;
+    c->dbg_delta_tilde = false;
     cudaEvent_t ev[6];
     for (int i = 0; i < 6; ++i) CU(cudaEventCreate(&ev[i]));
     double acc[5] = {0, 0, 0, 0, 0};
@@ -834,6 +933,7 @@ int lgf_profile_iterate(lgf_ctx* c, int64_t n, double alpha, double ms[5], lgf_r
         for (int k = 0; k < 5 && !rc; ++k) {
             CU(cudaEventRecord(ev[k], c->stream));
             if (k < 3) rc = DISPATCH(c, fft(c, k, true));
+            else if (c->fused_tile >= 0) { if (k == 3) rc = DISPATCH(c, k51(c, alpha)); }   // ms[4] stays ~0
             else if (k == 3) rc = DISPATCH(c, k5(c, alpha));
             else rc = DISPATCH(c, k1(c, 1));
         }
@@ -857,5 +957,14 @@ int lgf_profile_iterate(lgf_ctx* c, int64_t n, double alpha, double ms[5], lgf_r
 }
 
 int64_t lgf_launch_count(const lgf_ctx* c) { return c ? c->launches : 0; }
+
+int lgf_path_info(const lgf_ctx* c, int32_t info[4]) {
+    if (!c || !info) return LGF_EINVAL;
+    info[0] = c->xy_pipe ? 2 : (c->xy_ct ? 1 : 0);
+    info[1] = c->fused_tile >= 0 ? 1 : 0;
+    info[2] = c->fused_tile >= 0 ? c->fused_grid : c->lo.nblocks_site;
+    info[3] = c->launches_per_iter;
+    return LGF_OK;
+}
 
 }  // extern "C"

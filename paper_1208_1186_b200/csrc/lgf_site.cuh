@@ -26,6 +26,8 @@ struct DevState {
     unsigned int ticket;     // K1 block counter for the last-block reduction
     double tol;
     long long max_iter;
+    int cur;                 // which of the two link buffers holds the current field (fused path swaps them)
+    int pad_;
 };
 
 // Resident CTAs per SM each site kernel is compiled for (= register cap 65536 / (256 * n)); measured
@@ -150,11 +152,12 @@ k1_delta_theta_F(const Cx<T>* __restrict__ U, Cx<T>* __restrict__ D, double2* __
 
 // Second half of K1: one CTA sums the per-CTA (theta, F) partials in index order (deterministic, no
 // float atomics), publishes theta and F and, at the end of an iteration (mode 1), bumps the
-// iteration count and evaluates the stopping test on the device.  A separate tiny launch instead
+// iteration count and evaluates the stopping test on the device (mode 2: end of a FUSED iteration,
+// which additionally swaps the roles of the two link buffers).  A separate tiny launch instead
 // of a last-CTA ticket: the K1 CTAs then retire without a fence + atomic tail.
 __global__ void __launch_bounds__(256)
 k1_finish(const double2* __restrict__ partials, int n, DevState* st, double V, int mode) {
-    if (mode == 1 && *reinterpret_cast<volatile int*>(&st->done)) return;
+    if (mode >= 1 && *reinterpret_cast<volatile int*>(&st->done)) return;
     double a = 0.0, b = 0.0;
     for (int i = threadIdx.x; i < n; i += 256) {
         const double2 p = partials[i];
@@ -166,9 +169,10 @@ k1_finish(const double2* __restrict__ partials, int n, DevState* st, double V, i
         const double theta = a / (3.0 * V);
         st->theta = theta;
         st->F = b / (12.0 * V);
-        if (mode == 1) {
+        if (mode >= 1) {
             const long long it = st->iter + 1;
             st->iter = it;
+            if (mode == 2) st->cur ^= 1;     // fused update: the new links were written to the other buffer
             if (theta < st->tol || it >= st->max_iter) st->done = 1;
         }
     }

@@ -264,3 +264,29 @@ def test_generic_and_compile_time_fft_paths_agree(monkeypatch):
         gf.iterate(2, ALPHA)
         assert np.max(np.abs(_cplx(gf.store()) - ref)) <= 1e-12
         gf.close()
+
+
+@pytest.mark.parametrize("L", [(8, 8, 8, 8), (16, 16, 8, 8), (32, 8, 4, 8)])
+@pytest.mark.parametrize("prec,stor", MODES)
+def test_fused_update_kernel(monkeypatch, L, prec, stor):
+    """K5 + K1 fused into the marching kernel (LGF_FUSED=1): out-of-place update with swapped link
+    buffers; links after 1, 2 (odd/even buffer) and 5 iterations, theta/F and the fix count vs the oracle."""
+    monkeypatch.setenv("LGF_FUSED", "1")
+    U = gi.make_config(L, 31, 0.59)
+    gf = _fixer(L, prec, stor, U)
+    if L[0] in (8, 16, 32) and L[2] % 4 == 0:
+        assert gf.path_info()["fused"]
+    for n in (1, 2, 5):
+        ref, thh, Fh = oracle.iterate(L, U, n, ALPHA)
+        gf.load(gi.as_real(U))
+        r = gf.iterate(n, ALPHA)
+        assert r.iterations == n
+        assert np.max(np.abs(_cplx(gf.store()) - ref)) <= (1e-12 if n == 1 else 1e-11)
+        assert abs(r.theta - thh[n]) <= 1e-10 * thh[n] and abs(r.F - Fh[n]) <= 1e-12
+        m = gf.measure()                                   # stand-alone K1 on the swapped buffer agrees with the fused Delta
+        assert abs(m.theta - r.theta) <= 1e-12 * r.theta and abs(m.F - r.F) <= 1e-14
+    _, nfix, th, F, _, _ = oracle.fix(L, U, ALPHA, 1e-12, 5000)
+    gf.load(gi.as_real(U))
+    rf = gf.fix(ALPHA, 1e-12, 5000)
+    assert rf.iterations == nfix and rf.converged and abs(rf.F - F) <= 1e-10 * F
+    gf.close()

@@ -21,8 +21,8 @@ def test_workspace_bytes_host_logic():
     b18 = lgf.workspace_bytes((32, 32, 32, 32), lgf.LGF_F64, lgf.LGF_REAL18)
     b12 = lgf.workspace_bytes((32, 32, 32, 32), lgf.LGF_F64, lgf.LGF_REAL12)
     f18 = lgf.workspace_bytes((32, 32, 32, 32), lgf.LGF_F32, lgf.LGF_REAL18)
-    assert b18 - b12 == 4 * 6 * V * 8                      # 6 reals per link saved
-    assert b18 >= 4 * 18 * V * 8 + 8 * V * 8               # links + packed Delta
+    assert b18 - b12 == 2 * 4 * 6 * V * 8                  # 6 reals per link saved, in both link buffers
+    assert b18 >= 2 * 4 * 18 * V * 8 + 3 * 8 * V * 8       # two link buffers + Delta, Delta~, layout-B spectrum
     assert f18 < b18
     assert lgf.workspace_bytes((5, 8, 8, 8), lgf.LGF_F64, lgf.LGF_REAL18) == 0     # 5 is not 2^a 3^b
     assert lgf.workspace_bytes((1, 8, 8, 8), lgf.LGF_F64, lgf.LGF_REAL18) == 0
