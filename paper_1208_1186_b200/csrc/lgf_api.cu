@@ -373,7 +373,7 @@ struct Impl {
     }
     struct FusedEntry { int tx, ty, tz, threads; size_t smem; const void* kernel; };
     template <class Tile, int MINB> static FusedEntry fused_entry() {
-        return FusedEntry{Tile::TX, Tile::TY, Tile::TZ, Tile::NS, Tile::template smem_bytes<T>(),
+        return FusedEntry{Tile::TX, Tile::TY, Tile::TZ, Tile::NS, Tile::template smem_bytes<T, NC>(),
                           (const void*)&k51_update_delta<T, NC, Tile, MINB>};
     }
     static const FusedEntry* fused_entries() {
@@ -386,10 +386,11 @@ struct Impl {
             fused_entry<MarchTile<32, 4, 4>, 1>(),
             fused_entry<MarchTile<48, 4, 2>, 1>(),
             fused_entry<MarchTile<64, 4, 2>, 1>(),
+            fused_entry<MarchTile<32, 4, 2, true>, 1>(),
         };
         return tab;
     }
-    static constexpr int kNumFused = 8;
+    static constexpr int kNumFused = 9;
     // pick the marching tile for this lattice (LGF_FUSED = 0 disables the fused path, LGF_FUSED_TILE = i forces entry i)
     static int plan_fused(lgf_ctx* c) {
         c->fused_tile = -1;
@@ -401,6 +402,7 @@ struct Impl {
         for (int i = 0; i < kNumFused; ++i) {
             if (ft && atoi(ft) != i) continue;
             if (tab[i].tx != c->L[0] || c->L[1] % tab[i].ty || c->L[2] % tab[i].tz) continue;
+            if (tab[i].smem > (size_t)227 * 1024) continue;     // e.g. the staged tile in fp64 18-real
             c->fused_tile = i;
             break;
         }

@@ -27,13 +27,22 @@
 
 namespace lgf {
 
-template <int TX_, int TY_, int TZ_>
+template <int TX_, int TY_, int TZ_, bool STAGE_ = false>
 struct MarchTile {
     static constexpr int TX = TX_, TY = TY_, TZ = TZ_;
+    // STAGE: every thread keeps the links and the Delta~ it needs at the NEXT step in flight as
+    // cp.async copies into its own shared-memory slots (no registers, no barrier: a thread reads back
+    // only what it copied itself), so global latency is off the critical path of the march.
+    static constexpr bool kStage = STAGE_;
     static constexpr int NS = TX * TY * TZ;          // sites per t-slice of the tile = threads
-    static constexpr int HY = TX * TZ, HZ = TX * TY; // forward halo sites (y face, z face)
-    static constexpr int NG = NS + HY + HZ;          // g slots
-    template <typename T> static constexpr size_t smem_bytes() { return sizeof(Cx<T>) * (size_t)(9 * NG + 12 * NS); }
+    static constexpr int HY = TX * TZ, HZ = TX * TY; // halo sites of one y face / one z face
+    static constexpr int NG = NS + HY + HZ;          // g slots: the slice + its forward y and z halo
+    static constexpr int NH = HY + HZ;               // q slots of the backward halo links
+    static constexpr bool kShflX = (TX == 32);       // a warp is one x row: q_x travels by shuffle
+    static constexpr int NQ = kShflX ? 2 : 3;        // directions exchanged through shared memory
+    template <typename T, int NC> static constexpr size_t smem_bytes() {
+        return sizeof(Cx<T>) * (size_t)(9 * NG + 4 * NQ * NS + 4 * NH + (kStage ? (4 * NC + 4) * NS : 0));
+    }
 };
 
 struct MarchGeom {
@@ -91,7 +100,26 @@ __device__ __forceinline__ void store_link(const Su3<T>& u, Cx<T>* __restrict__ 
     for (int c = 0; c < NC; ++c) st_cx(p + (size_t)c * V, u.m[c]);
 }
 
-template <typename T, int NC> struct FusedOcc { static constexpr int value = 2; };
+
+// shuffle a complex number from lane `src` of the warp
+__device__ __forceinline__ Cx<double> shfl_cx(Cx<double> v, int src) {
+    return Cx<double>(__shfl_sync(0xffffffffu, v.re, src), __shfl_sync(0xffffffffu, v.im, src));
+}
+__device__ __forceinline__ Cx<float> shfl_cx(Cx<float> v, int src) {
+    return Cx<float>(__shfl_sync(0xffffffffu, v.re, src), __shfl_sync(0xffffffffu, v.im, src));
+}
+// per-thread asynchronous global -> shared copy of one complex number (LDGSTS), and its group fences
+__device__ __forceinline__ void cp_async_cx(Cx<double>* dst, const Cx<double>* src) {
+    asm volatile("cp.async.cg.shared.global [%0], [%1], 16;" ::"r"((uint32_t)__cvta_generic_to_shared(dst)), "l"(src) : "memory");
+}
+__device__ __forceinline__ void cp_async_cx(Cx<float>* dst, const Cx<float>* src) {
+    asm volatile("cp.async.ca.shared.global [%0], [%1], 8;" ::"r"((uint32_t)__cvta_generic_to_shared(dst)), "l"(src) : "memory");
+}
+__device__ __forceinline__ void cp_async_commit() { asm volatile("cp.async.commit_group;" ::: "memory"); }
+template <int N> __device__ __forceinline__ void cp_async_wait() { asm volatile("cp.async.wait_group %0;" ::"n"(N) : "memory"); }
+
+// pull the 128-byte line holding p towards L2 ahead of the next step's loads
+__device__ __forceinline__ void prefetch_l2(const void* p) { asm volatile("prefetch.global.L2 [%0];" ::"l"(p)); }
 
 template <typename T, int NC, class Tile, int MINB>
 __global__ void __launch_bounds__(Tile::NS, MINB)
@@ -99,9 +127,16 @@ k51_update_delta(const Cx<T>* __restrict__ U0, const Cx<T>* __restrict__ U1, con
                  Cx<T>* __restrict__ Dout, double2* __restrict__ partials, const DevState* st, MarchGeom g, T ha) {
     extern __shared__ __align__(16) unsigned char fused_smem[];
     if (*reinterpret_cast<const volatile int*>(&st->done)) return;
-    constexpr int TX = Tile::TX, TY = Tile::TY, TZ = Tile::TZ, NS = Tile::NS, NG = Tile::NG, NR = NC / 3;
-    Cx<T>* G = reinterpret_cast<Cx<T>*>(fused_smem);     // [9][NG]
-    Cx<T>* Q = G + 9 * NG;                               // [3][4][NS]
+    constexpr int TX = Tile::TX, TY = Tile::TY, TZ = Tile::TZ, NS = Tile::NS, NG = Tile::NG, NH = Tile::NH, NR = NC / 3;
+    constexpr int HY = Tile::HY;
+    constexpr bool SHX = Tile::kShflX;
+    constexpr int QY = SHX ? 0 : 1, QZ = SHX ? 1 : 2;   // planes of Q holding q_y, q_z (q_x in plane 0 unless shuffled)
+    Cx<T>* G = reinterpret_cast<Cx<T>*>(fused_smem);     // [9][NG]   g of the slice + forward halo
+    Cx<T>* Q = G + 9 * NG;                               // [NQ][4][NS]  q_mu of the slice
+    Cx<T>* QH = Q + 4 * Tile::NQ * NS;                   // [4][NH]   q of the backward halo links
+    constexpr bool STG = Tile::kStage;
+    Cx<T>* S = QH + 4 * NH;                              // [4*NC][NS] staged links of the step (STG)
+    Cx<T>* SD = S + 4 * NC * NS;                         // [4][NS]    staged Delta~(x+t) of the step (STG)
     const int cur = *reinterpret_cast<const volatile int*>(&st->cur);
     const Cx<T>* __restrict__ Uin = cur ? U1 : U0;
     Cx<T>* __restrict__ Uout = const_cast<Cx<T>*>(cur ? U0 : U1);
@@ -110,37 +145,70 @@ k51_update_delta(const Cx<T>* __restrict__ U0, const Cx<T>* __restrict__ U1, con
     const int lx = tid % TX, ly = (tid / TX) % TY, lz = tid / (TX * TY);
     const int Lx = g.L[0], Ly = g.L[1], Lz = g.L[2], Lt = g.L[3];
     const long long V = g.V, sy = Lx, sz = (long long)Lx * Ly, stt = sz * Lz;
-    // in-tile neighbours (x always wraps inside the tile; y/z wrap inside only if the tile spans the axis)
     const bool wrap_y = (Ly == TY), wrap_z = (Lz == TZ);
+    const int nhy = wrap_y ? 0 : HY, nh = nhy + (wrap_z ? 0 : Tile::HZ);     // halo items of this lattice
     const int fx = tid - lx + (lx + 1 == TX ? 0 : lx + 1), bx = tid - lx + (lx == 0 ? TX - 1 : lx - 1);
     const bool fy_in = (ly + 1 < TY) || wrap_y, by_in = (ly > 0) || wrap_y;
     const bool fz_in = (lz + 1 < TZ) || wrap_z, bz_in = (lz > 0) || wrap_z;
     const int fy = fy_in ? (ly + 1 < TY ? tid + TX : tid - TX * (TY - 1)) : NS + lx + TX * lz;
-    const int fz = fz_in ? (lz + 1 < TZ ? tid + TX * TY : tid - TX * TY * (TZ - 1)) : NS + Tile::HY + lx + TX * ly;
-    const int by = ly > 0 ? tid - TX : tid + TX * (TY - 1);
-    const int bz = lz > 0 ? tid - TX * TY : tid + TX * TY * (TZ - 1);
+    const int fz = fz_in ? (lz + 1 < TZ ? tid + TX * TY : tid - TX * TY * (TZ - 1)) : NS + HY + lx + TX * ly;
+    const int by = by_in ? (ly > 0 ? tid - TX : tid + TX * (TY - 1)) : lx + TX * lz;              // Q slot, or QH item
+    const int bz = bz_in ? (lz > 0 ? tid - TX * TY : tid + TX * TY * (TZ - 1)) : nhy + lx + TX * ly;
+    const long long sloc = lx + sy * ly + sz * lz;       // this thread's site relative to the tile origin
+    const bool pf_lane = (lx % (int)(128 / sizeof(Cx<T>))) == 0;
 
-    // this CTA's contiguous range of the slice sequence (column-major: tile column, then t)
     const long long q0 = g.nslices * (long long)blockIdx.x / gridDim.x;
     const long long q1 = g.nslices * (long long)(blockIdx.x + 1) / gridDim.x;
     double th = 0.0, fn = 0.0;
-    Cx<T> qtp[4];                       // q_t(x - t) carried from the previous step
-    long long sxyz = 0, yf_off = 0, zf_off = 0, yb_off = 0, zb_off = 0;
+    Cx<T> qtp[4];                       // q_t(x - t), carried from the previous step
+    long long s0 = 0, yf_off = 0, zf_off = 0, yb_off = 0, zb_off = 0;   // tile origin (t = 0) and face offsets
 
     auto own_g = [&](int c) { return G[c * NG + tid]; };
+    // halo item h -> site offset (relative to the slice's tile origin) of a y-face / z-face position
+    auto item_site = [&](int h, bool& is_y) -> long long {
+        is_y = h < nhy;
+        const int k = is_y ? h : h - nhy;
+        const int a = k % TX, b = k / TX;
+        return is_y ? a + sz * b : a + sy * b;
+    };
+
+    // STG: this thread's copies for slice index qq, batch b (0..2: link b; 3: link t and Delta~(x+t));
+    // one commit per batch, also when there is nothing left to copy, so that the group count stays 4 per step
+    auto stage_issue = [&](long long qq, int b) {
+        if (qq < q1) {
+            const int c2 = (int)(qq / Lt), t2 = (int)(qq - (long long)c2 * Lt);
+            const long long sn = sy * ((c2 % g.nby) * TY) + sz * ((c2 / g.nby) * TZ) + sloc + (long long)t2 * stt;
+#pragma unroll
+            for (int c = 0; c < NC; ++c) cp_async_cx(S + (b * NC + c) * NS + tid, Uin + (size_t)(b * NC + c) * V + sn);
+            if (b == 3) {
+                const long long sfn = sn + (t2 == Lt - 1 ? -(long long)(Lt - 1) * stt : stt);
+#pragma unroll
+                for (int c = 0; c < 4; ++c) cp_async_cx(SD + c * NS + tid, Dt + (size_t)c * V + sfn);
+            }
+        }
+        cp_async_commit();
+    };
+    auto staged_link = [&](Su3<T>& u, int b) {
+#pragma unroll
+        for (int c = 0; c < NC; ++c) u.m[c] = S[(b * NC + c) * NS + tid];
+        if (NC == 6) rebuild_row2(u);
+    };
+    if (STG) {
+#pragma unroll
+        for (int b = 0; b < 4; ++b) stage_issue(q0, b);
+    }
 
     for (long long q = q0; q < q1; ++q) {
         const int col = (int)(q / Lt), t = (int)(q - (long long)col * Lt);
         if (q == q0 || t == 0) {
-            // ---- new column (or first step): coordinates, g of the first slice, q_t of the slice behind ----
-            const int tby = col % g.nby, tbz = col / g.nby;
-            const int y = tby * TY + ly, z = tbz * TZ + lz;
-            sxyz = lx + sy * y + sz * z;
-            yf_off = (y + 1 == Ly) ? -(long long)(Ly - 1) * sy : sy;
-            yb_off = (y == 0) ? (long long)(Ly - 1) * sy : -sy;
-            zf_off = (z + 1 == Lz) ? -(long long)(Lz - 1) * sz : sz;
-            zb_off = (z == 0) ? (long long)(Lz - 1) * sz : -sz;
-            const long long s = sxyz + (long long)t * stt;
+            // ---- new column (or first step): tile origin, g of the first slice, q_t of the slice behind ----
+            const int y0 = (col % g.nby) * TY, z0 = (col / g.nby) * TZ;
+            s0 = sy * y0 + sz * z0;
+            yf_off = (long long)((y0 + TY) % Ly - y0) * sy;
+            yb_off = (long long)((y0 + Ly - 1) % Ly - y0) * sy;
+            zf_off = (long long)((z0 + TZ) % Lz - z0) * sz;
+            zb_off = (long long)((z0 + Lz - 1) % Lz - z0) * sz;
+            const long long s = s0 + sloc + (long long)t * stt;
             const long long sb = s + (t == 0 ? (long long)(Lt - 1) * stt : -stt);
             Su3<T> g0, gb, u, un;
             load_g(g0, Dt, V, s, ha);
@@ -148,80 +216,106 @@ k51_update_delta(const Cx<T>* __restrict__ U0, const Cx<T>* __restrict__ U1, con
             load_link<T, NC>(u, Uin, V, 3, sb);
             sandwich<T, NR>(un, u, [&](int c) { return gb.m[c]; }, [&](int c) { return g0.m[c]; });
             project_ah(un, qtp);
-            __syncthreads();            // the previous column's last reads of G are done
+            __syncthreads();            // uniform branch; the previous column is completely done
 #pragma unroll
             for (int c = 0; c < 9; ++c) G[c * NG + tid] = g0.m[c];
         }
-        const long long s = sxyz + (long long)t * stt;
-        // ---- (1) forward halo g's of this slice, built by the face rows ----
-        if (!fy_in) {
+        const long long sbase = s0 + (long long)t * stt;
+        const long long s = sbase + sloc;
+        // ---- (1) forward halo g's of this slice, one item per thread ----
+        for (int h = tid; h < nh; h += NS) {
+            bool is_y;
+            const long long hs = sbase + item_site(h, is_y) + (is_y ? yf_off : zf_off);
             Su3<T> gh;
-            load_g(gh, Dt, V, s + yf_off, ha);
+            load_g(gh, Dt, V, hs, ha);
+            const int slot = NS + (is_y ? h : HY + (h - nhy));
 #pragma unroll
-            for (int c = 0; c < 9; ++c) G[c * NG + fy] = gh.m[c];
+            for (int c = 0; c < 9; ++c) G[c * NG + slot] = gh.m[c];
         }
-        if (!fz_in) {
-            Su3<T> gh;
-            load_g(gh, Dt, V, s + zf_off, ha);
+        // next slice's lines towards L2 while this one is being worked on
+        if (!STG && pf_lane && t + 1 < Lt) {
 #pragma unroll
-            for (int c = 0; c < 9; ++c) G[c * NG + fz] = gh.m[c];
+            for (int mu = 0; mu < 4; ++mu)
+#pragma unroll
+                for (int c = 0; c < NC; ++c) prefetch_l2(Uin + (size_t)(mu * NC + c) * V + s + stt);
+            if (t + 2 < Lt) {
+#pragma unroll
+                for (int c = 0; c < 4; ++c) prefetch_l2(Dt + (size_t)c * V + s + 2 * stt);
+            }
         }
         __syncthreads();                // (a) g of the slice and of its forward halo is in place
         Cx<T> acc[4] = {qtp[0], qtp[1], qtp[2], qtp[3]};
         T retr = 0;
-        // ---- (2) links mu = x, y, z ----
+        // ---- (2) links mu = x, y, z of this site ----
 #pragma unroll
         for (int mu = 0; mu < 3; ++mu) {
             const int f = mu == 0 ? fx : (mu == 1 ? fy : fz);
             Su3<T> u, un;
-            load_link<T, NC>(u, Uin, V, mu, s);
+            if (STG) {
+                cp_async_wait<3>();                 // the batch issued one step ago has landed
+                staged_link(u, mu);
+                stage_issue(q + 1, mu);             // same slots, next slice
+            } else {
+                load_link<T, NC>(u, Uin, V, mu, s);
+            }
             sandwich<T, NR>(un, u, own_g, [&](int c) { return G[c * NG + f]; });
             store_link<T, NC>(un, Uout, V, mu, s);
             retr += un.m[0].re + un.m[4].re + un.m[8].re;
             Cx<T> qq[4];
             project_ah(un, qq);
+            if (SHX && mu == 0) {
+                // the warp is this x row: q_x(x - 1) comes from the lane to the left (periodic)
 #pragma unroll
-            for (int c = 0; c < 4; ++c) {
-                acc[c] = acc[c] - qq[c];
-                Q[(mu * 4 + c) * NS + tid] = qq[c];
+                for (int c = 0; c < 4; ++c) acc[c] = (acc[c] - qq[c]) + shfl_cx(qq[c], (lx + 31) & 31);
+            } else {
+                const int plane = mu == 0 ? 0 : (mu == 1 ? QY : QZ);
+#pragma unroll
+                for (int c = 0; c < 4; ++c) {
+                    acc[c] = acc[c] - qq[c];
+                    Q[(plane * 4 + c) * NS + tid] = qq[c];
+                }
             }
         }
-        __syncthreads();                // (b) q_mu of the slice is in place; nobody reads G's neighbours any more
-        // ---- (3) backward contributions ----
-#pragma unroll
-        for (int c = 0; c < 4; ++c) acc[c] = acc[c] + Q[(0 * 4 + c) * NS + bx];
-        if (by_in) {
-#pragma unroll
-            for (int c = 0; c < 4; ++c) acc[c] = acc[c] + Q[(1 * 4 + c) * NS + by];
-        } else {
+        // ---- backward halo links (owned by the neighbouring tiles), one item per thread ----
+        for (int h = tid; h < nh; h += NS) {
+            bool is_y;
+            const long long loc = item_site(h, is_y);
+            const long long hs = sbase + loc + (is_y ? yb_off : zb_off);
+            // the face site this link ends on: (a, 0, b) for a y item, (a, b, 0) for a z item
+            const int k = is_y ? h : h - nhy;
+            const int ts = is_y ? (k % TX) + TX * TY * (k / TX) : k;
             Su3<T> gb, u, un;
-            load_g(gb, Dt, V, s + yb_off, ha);
-            load_link<T, NC>(u, Uin, V, 1, s + yb_off);
-            sandwich<T, NR>(un, u, [&](int c) { return gb.m[c]; }, own_g);
+            load_g(gb, Dt, V, hs, ha);
+            load_link<T, NC>(u, Uin, V, is_y ? 1 : 2, hs);
+            sandwich<T, NR>(un, u, [&](int c) { return gb.m[c]; }, [&](int c) { return G[c * NG + ts]; });
             Cx<T> qq[4];
             project_ah(un, qq);
 #pragma unroll
-            for (int c = 0; c < 4; ++c) acc[c] = acc[c] + qq[c];
+            for (int c = 0; c < 4; ++c) QH[c * NH + h] = qq[c];
         }
-        if (bz_in) {
+        __syncthreads();                // (b) q_mu of the slice and of the halo links is in place
+        // ---- (3) backward contributions, then the t link ----
+        if (!SHX) {
 #pragma unroll
-            for (int c = 0; c < 4; ++c) acc[c] = acc[c] + Q[(2 * 4 + c) * NS + bz];
-        } else {
-            Su3<T> gb, u, un;
-            load_g(gb, Dt, V, s + zb_off, ha);
-            load_link<T, NC>(u, Uin, V, 2, s + zb_off);
-            sandwich<T, NR>(un, u, [&](int c) { return gb.m[c]; }, own_g);
-            Cx<T> qq[4];
-            project_ah(un, qq);
-#pragma unroll
-            for (int c = 0; c < 4; ++c) acc[c] = acc[c] + qq[c];
+            for (int c = 0; c < 4; ++c) acc[c] = acc[c] + Q[(0 * 4 + c) * NS + bx];
         }
-        // ---- link mu = t: g(x+t) is built here and becomes the next step's g ----
+#pragma unroll
+        for (int c = 0; c < 4; ++c) acc[c] = acc[c] + (by_in ? Q[(QY * 4 + c) * NS + by] : QH[c * NH + by]);
+#pragma unroll
+        for (int c = 0; c < 4; ++c) acc[c] = acc[c] + (bz_in ? Q[(QZ * 4 + c) * NS + bz] : QH[c * NH + bz]);
         {
+            // g(x+t) is built here and becomes the next step's g
             const long long sf = s + (t == Lt - 1 ? -(long long)(Lt - 1) * stt : stt);
             Su3<T> gt, u, un;
-            load_g(gt, Dt, V, sf, ha);
-            load_link<T, NC>(u, Uin, V, 3, s);
+            if (STG) {
+                cp_async_wait<3>();
+                build_g(gt, SD[tid], SD[NS + tid], SD[2 * NS + tid], SD[3 * NS + tid], ha);
+                staged_link(u, 3);
+                stage_issue(q + 1, 3);
+            } else {
+                load_g(gt, Dt, V, sf, ha);
+                load_link<T, NC>(u, Uin, V, 3, s);
+            }
             sandwich<T, NR>(un, u, own_g, [&](int c) { return gt.m[c]; });
             store_link<T, NC>(un, Uout, V, 3, s);
             retr += un.m[0].re + un.m[4].re + un.m[8].re;
@@ -229,7 +323,7 @@ k51_update_delta(const Cx<T>* __restrict__ U0, const Cx<T>* __restrict__ U1, con
 #pragma unroll
             for (int c = 0; c < 4; ++c) acc[c] = acc[c] - qtp[c];
 #pragma unroll
-            for (int c = 0; c < 9; ++c) G[c * NG + tid] = gt.m[c];     // own slot: read by others only after the next (a)
+            for (int c = 0; c < 9; ++c) G[c * NG + tid] = gt.m[c];     // own slot: others read it only after the next (a)
         }
         // ---- Delta', theta, F of the new links at this site ----
         st_cx(Dout + s, acc[0]);
