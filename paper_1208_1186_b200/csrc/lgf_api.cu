@@ -52,6 +52,14 @@ const int kSiteTileDims[kNumSiteTiles][4] = {{8, 4, 4, 2}, {16, 4, 2, 2}, {32, 2
 typedef SiteTileMu<8, 4, 2, 1> TileM0;
 typedef SiteTileMu<32, 2, 1, 1> TileM1;
 typedef SiteTileMu<16, 4, 1, 1> TileM2;
+// shared-g K5 (k5s): sites per CTA x 4 directions
+typedef SiteTileS<8, 2, 2, 2> TileS0;
+typedef SiteTileS<8, 4, 2, 2> TileS1;
+typedef SiteTileS<16, 2, 2, 1> TileS2;
+typedef SiteTileS<32, 2, 1, 1> TileS3;
+typedef SiteTileS<16, 2, 2, 2> TileS4;
+constexpr int kNumSTiles = 5;
+const int kSTileDims[kNumSTiles][4] = {{8, 2, 2, 2}, {8, 4, 2, 2}, {16, 2, 2, 1}, {32, 2, 1, 1}, {16, 2, 2, 2}};
 constexpr int kNumMuTiles = 3;
 const int kMuTileDims[kNumMuTiles][4] = {{8, 4, 2, 1}, {32, 2, 1, 1}, {16, 4, 1, 1}};
 constexpr int kStageSites = 1 << 15;       // boundary staging chunk (sites)
@@ -139,6 +147,9 @@ struct lgf_ctx {
     int site_variant;            // 0: thread per (site, direction); 1: thread per site
     int site_tile;               // index into kSiteTileDims for the thread-per-site kernels
     int mu_tile;                 // index into kMuTileDims for k5m
+    int s_tile;                  // index into kSTileDims for k5s (site_variant 2)
+    Geom geom_s;
+    int nblocks_s;
     Axis axis[4];
     XyPass xy;                   // K2, K4
     ZtPass zt;                   // K3
@@ -426,6 +437,19 @@ struct Impl {
         return LGF_OK;
     }
     static int k5(lgf_ctx* c, double alpha) {
+        if (c->site_variant == 2) {
+#define LGF_K5S_CASE(ID, TILE, MINB) case ID: k5s_gbuild_update<T, NC, TILE, MINB><<<c->nblocks_s, TILE::kThreads, 0, c->stream>>>( \
+                links(c), delta(c), dev_state(c), c->geom_s, (T)(0.5 * alpha)); break;
+            switch (c->s_tile) {
+                LGF_K5S_CASE(1, TileS1, 1) LGF_K5S_CASE(2, TileS2, 2) LGF_K5S_CASE(3, TileS3, 2) LGF_K5S_CASE(4, TileS4, 1)
+                default: k5s_gbuild_update<T, NC, TileS0, 2><<<c->nblocks_s, TileS0::kThreads, 0, c->stream>>>(
+                    links(c), delta(c), dev_state(c), c->geom_s, (T)(0.5 * alpha));
+            }
+#undef LGF_K5S_CASE
+            c->launches++;
+            CU(cudaGetLastError());
+            return LGF_OK;
+        }
         if (c->site_variant == 0) {
 #define LGF_K5M_CASE(ID, TILE) case ID: k5m_gbuild_update<T, NC, TILE><<<c->lo.nblocks_mu, TILE::kThreads, 0, c->stream>>>( \
                 links(c), delta(c), dev_state(c), c->geom_mu, (T)(0.5 * alpha)); break;
@@ -710,7 +734,9 @@ static int create_common(const int32_t L[4], int precision, int storage, void* w
         const char* e = getenv("LGF_SITE_VARIANT");
         // measured at 32^4: the (site, direction) split wins for fp64 18-real and fp32 12-real
         const bool mu_default = (precision == LGF_F64 && storage == LGF_REAL18) || (precision == LGF_F32 && storage == LGF_REAL12);
-        c->site_variant = e ? atoi(e) : (mu_default ? 0 : 1);
+        // measured at 32^4: the shared-g (site, direction) kernel k5s wins for fp64 18-real (233 vs 247 us) and
+        // fp32 12-real (102 vs 107 us); thread-per-site wins for fp64 12-real (175 vs 194 us) and fp32 18-real
+        c->site_variant = e ? atoi(e) : (mu_default ? 2 : 1);
         int t = (L[0] % 16 == 0) ? 2 : 0;
         e = getenv("LGF_SITEMU_TILE");
         if (e && atoi(e) >= 0 && atoi(e) < kNumMuTiles) t = atoi(e);
@@ -721,6 +747,24 @@ static int create_common(const int32_t L[4], int precision, int storage, void* w
     }
     c->geom_mu = c->geom;
     for (int i = 0; i < 4; ++i) c->geom_mu.nb[i] = c->lo.nbm[i];
+    const int mu_default_fallback = ((precision == LGF_F64 && storage == LGF_REAL18) || (precision == LGF_F32 && storage == LGF_REAL12)) ? 0 : 1;
+    {   // shared-g K5 (LGF_SITE_VARIANT=2, LGF_SITES_TILE): needs every extent to be a multiple of the tile's
+        const char* e = getenv("LGF_SITES_TILE");
+        int t = (e && atoi(e) >= 0 && atoi(e) < kNumSTiles) ? atoi(e) : (precision == LGF_F64 ? 2 : 3);
+        for (int k = 0; k < 4 && !e; ++k)               // default tile does not divide the lattice: try the smallest one
+            if (L[k] % kSTileDims[t][k]) { t = 0; break; }
+        c->s_tile = t;
+        c->geom_s = c->geom;
+        int n = 1;
+        bool ok = true;
+        for (int i = 0; i < 4; ++i) {
+            ok = ok && (L[i] % kSTileDims[t][i] == 0);
+            c->geom_s.nb[i] = L[i] / kSTileDims[t][i];
+            n *= c->geom_s.nb[i] > 0 ? c->geom_s.nb[i] : 1;
+        }
+        c->nblocks_s = n;
+        if (c->site_variant == 2 && !ok) c->site_variant = mu_default_fallback;
+    }
     int rc = LGF_OK;
     if (ws_bytes < c->lo.total || (reinterpret_cast<uintptr_t>(ws) % kAlign) != 0) rc = LGF_EINVAL;
     if (!rc && !plan_passes(c)) rc = LGF_EUNSUPPORTED;

@@ -31,5 +31,18 @@ struct ZtP {
     }
 };
 
+// half-tile ring variant of K3 (fft_zt_pipe_halves): three half-tile buffers
+template <typename T, int NZ, int Z1, int NT, int T1, int CX, int GT>
+struct ZtPH {
+    typedef LineSplit<NZ, Z1> SZ;
+    typedef LineSplit<NT, T1> ST_;
+    static constexpr size_t kSmem = sizeof(Cx<T>) * (size_t)3 * CX * (NZ + 1) * (NT / 2) + 8 * 3;
+    static_assert(kSmem <= 227 * 1024, "half-tile ring exceeds shared memory");
+    static_assert((CX & (CX - 1)) == 0, "CX must be a power of two");
+    static ZtPipeEntry entry() {
+        return ZtPipeEntry{NZ, NT, CX, GT, 3, kSmem, (const void*)&fft_zt_pipe_halves<T, SZ, ST_, CX, GT>};
+    }
+};
+
 }  // namespace pinst
 }  // namespace lgf

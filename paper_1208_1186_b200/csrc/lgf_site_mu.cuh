@@ -87,4 +87,91 @@ k5m_gbuild_update(Cx<T>* __restrict__ U, const Cx<T>* __restrict__ D, const DevS
         }
 }
 
+// ---------------------------------------------------------------------------------------------
+// K5, thread (site, mu) with g shared through shared memory: every g of the tile and of its four
+// forward halo faces is built ONCE by one thread (instead of 5-8 times per site), the link loads
+// are issued before the g phase so that they overlap it, and a single barrier separates the two.
+// Requires every L_mu to be a multiple of the tile extent (no ragged tiles).
+// ---------------------------------------------------------------------------------------------
+template <int TX, int TY, int TZ, int TT>
+struct SiteTileS {
+    static constexpr int tx = TX, ty = TY, tz = TZ, tt = TT;
+    static constexpr int kSites = TX * TY * TZ * TT;
+    static constexpr int kThreads = 4 * kSites;
+    static constexpr int HX = TY * TZ * TT, HY = TX * TZ * TT, HZ = TX * TY * TT, HT = TX * TY * TZ;
+    static constexpr int OX = kSites, OY = OX + HX, OZ = OY + HY, OT = OZ + HZ, NG = OT + HT;   // g slots
+    static_assert(kSites % 32 == 0, "mu must be warp-uniform");
+};
+
+template <typename T, int NC, class Tile, int MINB>
+__global__ void __launch_bounds__(Tile::kThreads, MINB)
+k5s_gbuild_update(Cx<T>* __restrict__ U, const Cx<T>* __restrict__ D, const DevState* st, Geom g, T half_alpha) {
+    if (*reinterpret_cast<const volatile int*>(&st->done)) return;
+    constexpr int TX = Tile::tx, TY = Tile::ty, TZ = Tile::tz, TT = Tile::tt, NS = Tile::kSites, NG = Tile::NG, NR = NC / 3;
+    __shared__ Cx<T> G[9 * NG];
+    int b = blockIdx.x;
+    const int x0 = (b % g.nb[0]) * TX; b /= g.nb[0];
+    const int y0 = (b % g.nb[1]) * TY; b /= g.nb[1];
+    const int z0 = (b % g.nb[2]) * TZ; b /= g.nb[2];
+    const int t0 = b * TT;
+    const long long s1 = g.L[0], s2 = s1 * g.L[1], s3 = s2 * g.L[2];
+    const int tid = threadIdx.x, ls = tid % NS, mu = tid / NS;
+    const int lx = ls % TX, ly = (ls / TX) % TY, lz = (ls / (TX * TY)) % TZ, lt = ls / (TX * TY * TZ);
+    const long long s = (x0 + lx) + s1 * (y0 + ly) + s2 * (z0 + lz) + s3 * (t0 + lt);
+    // ---- this thread's link: loads in flight during the whole g phase ----
+    Su3<T> u;
+    Cx<T>* p = U + (size_t)mu * NC * g.V + s;
+#pragma unroll
+    for (int c = 0; c < NC; ++c) u.m[c] = ld_cx(p + (size_t)c * g.V);
+    // ---- g of the tile and of its forward halo faces, one item per thread ----
+    for (int i = tid; i < NG; i += Tile::kThreads) {
+        int ax, ay, az, at;           // local coordinates of the item's site (may equal the tile extent: halo)
+        if (i < Tile::OX) { ax = i % TX; ay = (i / TX) % TY; az = (i / (TX * TY)) % TZ; at = i / (TX * TY * TZ); }
+        else if (i < Tile::OY) { const int h = i - Tile::OX; ax = TX; ay = h % TY; az = (h / TY) % TZ; at = h / (TY * TZ); }
+        else if (i < Tile::OZ) { const int h = i - Tile::OY; ax = h % TX; ay = TY; az = (h / TX) % TZ; at = h / (TX * TZ); }
+        else if (i < Tile::OT) { const int h = i - Tile::OZ; ax = h % TX; ay = h / TX % TY; az = TZ; at = h / (TX * TY); }
+        else { const int h = i - Tile::OT; ax = h % TX; ay = (h / TX) % TY; az = h / (TX * TY); at = TT; }
+        int gx = x0 + ax, gy = y0 + ay, gz = z0 + az, gt = t0 + at;
+        if (gx >= g.L[0]) gx -= g.L[0];
+        if (gy >= g.L[1]) gy -= g.L[1];
+        if (gz >= g.L[2]) gz -= g.L[2];
+        if (gt >= g.L[3]) gt -= g.L[3];
+        Su3<T> gg;
+        load_g(gg, D, g.V, gx + s1 * gy + s2 * gz + s3 * gt, half_alpha);
+#pragma unroll
+        for (int c = 0; c < 9; ++c) G[c * NG + i] = gg.m[c];
+    }
+    __syncthreads();
+    // ---- U' = g(x) U g(x+mu)^+ ----
+    int f;
+    if (mu == 0) f = lx + 1 < TX ? ls + 1 : Tile::OX + ly + TY * (lz + TZ * lt);
+    else if (mu == 1) f = ly + 1 < TY ? ls + TX : Tile::OY + lx + TX * (lz + TZ * lt);
+    else if (mu == 2) f = lz + 1 < TZ ? ls + TX * TY : Tile::OZ + lx + TX * (ly + TY * lt);
+    else f = lt + 1 < TT ? ls + TX * TY * TZ : Tile::OT + lx + TX * (ly + TY * lz);
+    if (NC == 6) rebuild_row2(u);
+    Cx<T> W[3 * NR];
+#pragma unroll
+    for (int i = 0; i < NR; ++i) {
+        const Cx<T> a0 = G[(3 * i) * NG + ls], a1 = G[(3 * i + 1) * NG + ls], a2 = G[(3 * i + 2) * NG + ls];
+#pragma unroll
+        for (int j = 0; j < 3; ++j) {
+            Cx<T> acc = a0 * u.m[j];
+            fma_cx(acc, a1, u.m[3 + j]);
+            fma_cx(acc, a2, u.m[6 + j]);
+            W[3 * i + j] = acc;
+        }
+    }
+#pragma unroll
+    for (int j = 0; j < 3; ++j) {
+        const Cx<T> b0 = G[(3 * j) * NG + f], b1 = G[(3 * j + 1) * NG + f], b2 = G[(3 * j + 2) * NG + f];
+#pragma unroll
+        for (int i = 0; i < NR; ++i) {
+            Cx<T> acc = mulc(W[3 * i], b0);
+            fma_cxc(acc, W[3 * i + 1], b1);
+            fma_cxc(acc, W[3 * i + 2], b2);
+            st_cx(p + (size_t)(3 * i + j) * g.V, acc);
+        }
+    }
+}
+
 }  // namespace lgf

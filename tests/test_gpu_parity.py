@@ -290,3 +290,25 @@ def test_fused_update_kernel(monkeypatch, L, prec, stor):
     rf = gf.fix(ALPHA, 1e-12, 5000)
     assert rf.iterations == nfix and rf.converged and abs(rf.F - F) <= 1e-10 * F
     gf.close()
+
+
+@pytest.mark.parametrize("L", [(8, 8, 64, 64), (64, 64, 8, 8), (48, 48, 8, 8), (8, 8, 48, 8)])
+def test_large_extent_fft_kernels(L):
+    """The 48- and 64-point two-stage line kernels (64^4's K3 runs on the half-tile ring) on lattices the
+    oracle still finishes in seconds: two iterations in fp64 12-real and fp32 18-real."""
+    U = gi.make_config(L, 33, 0.59)
+    ref, thh, Fh = oracle.iterate(L, U, 2, ALPHA)
+    gf = _fixer(L, lgf.LGF_F64, lgf.LGF_REAL12, U)
+    assert gf.path_info()["fft_path"] == "pipelined"
+    r = gf.iterate(2, ALPHA)
+    assert np.max(np.abs(_cplx(gf.store()) - ref)) <= 1e-12
+    assert abs(r.theta - thh[2]) <= 1e-10 * thh[2] and abs(r.F - Fh[2]) <= 1e-12
+    gf.close()
+    U32 = gi.as_real(U, torch.float32)
+    ref32, _, Fh32 = oracle.iterate(L, gi.from_real(U32), 2, ALPHA)
+    gf = lgf.GaugeFixer(L, lgf.LGF_F32, lgf.LGF_REAL18)
+    gf.load(U32)
+    r = gf.iterate(2, ALPHA)
+    assert np.max(np.abs(_cplx(gf.store()) - ref32)) <= 2e-5
+    assert abs(r.F - Fh32[2]) <= 1e-5 * abs(Fh32[2])
+    gf.close()
