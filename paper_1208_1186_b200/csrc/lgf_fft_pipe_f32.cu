@@ -10,6 +10,7 @@ const XyPipeEntry* xy_pipe_table_f32(int* n) {
     static const XyPipeEntry tab[] = {
         XyP<T, 8, 8, 8, 8, 16, 128, 2, 3>::entry(),
         XyP<T, 16, 16, 16, 16, 8, 128, 2, 3>::entry(),
+        XyP<T, 32, 32, 32, 32, 4, 128, 4, 6>::entry(),
         XyP<T, 32, 32, 32, 32, 4, 128, 2, 4>::entry(),
         XyP<T, 32, 32, 32, 32, 8, 256, 2, 3>::entry(),
         XyP<T, 48, 8, 48, 8, 2, 192, 2, 4>::entry(),
@@ -23,6 +24,7 @@ const ZtPipeEntry* zt_pipe_table_f32(int* n) {
     static const ZtPipeEntry tab[] = {
         ZtP<T, 8, 8, 8, 8, 8, 64, 2, 3>::entry(),
         ZtP<T, 16, 16, 16, 16, 8, 128, 2, 3>::entry(),
+        ZtP<T, 32, 32, 32, 32, 4, 128, 4, 6>::entry(),
         ZtP<T, 32, 32, 32, 32, 4, 128, 2, 4>::entry(),
         ZtP<T, 32, 32, 32, 32, 8, 256, 2, 3>::entry(),
         ZtP<T, 48, 8, 8, 8, 8, 128, 3, 4>::entry(),

@@ -12,6 +12,7 @@ const XyPipeEntry* xy_pipe_table_f64(int* n) {
         XyP<T, 16, 16, 16, 16, 8, 128, 2, 3>::entry(),
         XyP<T, 32, 32, 32, 32, 4, 128, 2, 3>::entry(),
         XyP<T, 32, 32, 32, 32, 2, 64, 4, 6>::entry(),
+        XyP<T, 32, 32, 32, 32, 4, 128, 3, 3>::entry(),
         XyP<T, 48, 8, 48, 8, 2, 192, 2, 3>::entry(),     // 576 / 768 items per stage: whole rounds of 192 threads
         XyP<T, 48, 8, 48, 8, 1, 256, 2, 4>::entry(),
         XyP<T, 64, 8, 64, 8, 1, 256, 2, 3>::entry(),
@@ -25,6 +26,7 @@ const ZtPipeEntry* zt_pipe_table_f64(int* n) {
         ZtP<T, 16, 16, 16, 16, 4, 64, 2, 3>::entry(),
         ZtP<T, 32, 32, 32, 32, 4, 128, 2, 3>::entry(),
         ZtP<T, 32, 32, 32, 32, 2, 64, 4, 6>::entry(),
+        ZtP<T, 32, 32, 32, 32, 4, 128, 3, 3>::entry(),
         ZtP<T, 48, 8, 8, 8, 8, 128, 3, 4>::entry(),        // 384 / 512 / 384 items: whole rounds of 128 threads
         ZtP<T, 48, 8, 8, 8, 8, 256, 2, 4>::entry(),
         ZtPH<T, 64, 8, 64, 8, 2, 512>::entry(),

@@ -68,6 +68,50 @@ template <typename T> __device__ __forceinline__ void st_cx(Cx<T>* p, Cx<T> a) {
     *reinterpret_cast<V*>(p) = v;
 }
 
+// Link traffic is streamed (each link is touched once per kernel): an L2 evict-first policy keeps the
+// 126 MB L2 for the Delta field, which K1 -> K2 -> K3 -> K4 -> K5 hand to each other.
+// LGF_STREAM_LINKS (compile-time, default 1) switches the hint off for A/B runs.
+#ifndef LGF_STREAM_LINKS
+#define LGF_STREAM_LINKS 1
+#endif
+__device__ __forceinline__ uint64_t l2_evict_first_policy() {
+    uint64_t p;
+    asm("createpolicy.fractional.L2::evict_first.b64 %0, 1.0;" : "=l"(p));
+    return p;
+}
+__device__ __forceinline__ Cx<double> ld_cx_stream(const Cx<double>* p, uint64_t pol) {
+#if LGF_STREAM_LINKS
+    double x, y;
+    asm("ld.global.L2::cache_hint.v2.f64 {%0, %1}, [%2], %3;" : "=d"(x), "=d"(y) : "l"(p), "l"(pol));
+    return Cx<double>(x, y);
+#else
+    return ld_cx(p);
+#endif
+}
+__device__ __forceinline__ Cx<float> ld_cx_stream(const Cx<float>* p, uint64_t pol) {
+#if LGF_STREAM_LINKS
+    float x, y;
+    asm("ld.global.L2::cache_hint.v2.f32 {%0, %1}, [%2], %3;" : "=f"(x), "=f"(y) : "l"(p), "l"(pol));
+    return Cx<float>(x, y);
+#else
+    return ld_cx(p);
+#endif
+}
+__device__ __forceinline__ void st_cx_stream(Cx<double>* p, Cx<double> a, uint64_t pol) {
+#if LGF_STREAM_LINKS
+    asm volatile("st.global.L2::cache_hint.v2.f64 [%0], {%1, %2}, %3;" ::"l"(p), "d"(a.re), "d"(a.im), "l"(pol) : "memory");
+#else
+    st_cx(p, a);
+#endif
+}
+__device__ __forceinline__ void st_cx_stream(Cx<float>* p, Cx<float> a, uint64_t pol) {
+#if LGF_STREAM_LINKS
+    asm volatile("st.global.L2::cache_hint.v2.f32 [%0], {%1, %2}, %3;" ::"l"(p), "f"(a.re), "f"(a.im), "l"(pol) : "memory");
+#else
+    st_cx(p, a);
+#endif
+}
+
 // 3x3 complex matrix in registers, row-major m[3*row + col]
 template <typename T> struct Su3 { Cx<T> m[9]; };
 

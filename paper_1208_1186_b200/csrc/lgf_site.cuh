@@ -67,11 +67,18 @@ __device__ __forceinline__ long long axis_stride(const Geom& g, int mu) {
 }
 
 // Load one link into registers; in 12-real mode rebuild row 2.
-template <typename T, int NC>
+// STREAM: this is the last use of the link in the kernel (L2 evict-first); otherwise a plain load.
+template <typename T, int NC, bool STREAM = false>
 __device__ __forceinline__ void load_link(Su3<T>& u, const Cx<T>* __restrict__ U, long long V, int mu, long long s) {
     const Cx<T>* p = U + (size_t)mu * NC * V + s;
+    if (STREAM) {
+        const uint64_t pol = l2_evict_first_policy();
 #pragma unroll
-    for (int c = 0; c < NC; ++c) u.m[c] = ld_cx(p + (size_t)c * V);
+        for (int c = 0; c < NC; ++c) u.m[c] = ld_cx_stream(p + (size_t)c * V, pol);
+    } else {
+#pragma unroll
+        for (int c = 0; c < NC; ++c) u.m[c] = ld_cx(p + (size_t)c * V);
+    }
     if (NC == 6) rebuild_row2(u);
 }
 
@@ -124,8 +131,10 @@ k1_delta_theta_F(const Cx<T>* __restrict__ U, Cx<T>* __restrict__ D, double2* __
         for (int mu = 0; mu < 4; ++mu) {
             const long long sb = (x[mu] == 0) ? s + stride * (g.L[mu] - 1) : s - stride;
             Su3<T> a, b;
-            load_link<T, NC>(a, U, g.V, mu, s);
-            load_link<T, NC>(b, U, g.V, mu, sb);
+            // measured at 32^4: evict-first link loads help K1 in fp32 (80 -> 69 us, the Delta it writes stays in
+            // L2 for K2) and hurt in fp64 (122 -> 134 us, 18-real: the backward re-reads start missing L2)
+            load_link<T, NC, sizeof(T) == 4>(a, U, g.V, mu, s);
+            load_link<T, NC, sizeof(T) == 4>(b, U, g.V, mu, sb);
 #pragma unroll
             for (int c = 0; c < 9; ++c) M.m[c] = M.m[c] + (b.m[c] - a.m[c]);
             retr += a.m[0].re + a.m[4].re + a.m[8].re;
