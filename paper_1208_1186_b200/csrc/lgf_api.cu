@@ -107,6 +107,11 @@ Layout make_layout(const int32_t L[4], int precision, int storage) {
         for (int i = 0; i < 4; ++i) n *= (size_t)((L[i] + kSiteTileDims[t][i] - 1) / kSiteTileDims[t][i]);
         if (n > nb) nb = n;
     }
+    for (int t = 0; t < kNumSTiles; ++t) {     // the (site, direction) tilings have fewer sites per CTA
+        size_t n = 1;
+        for (int i = 0; i < 4; ++i) n *= (size_t)((L[i] + kSTileDims[t][i] - 1) / kSTileDims[t][i]);
+        if (n > nb) nb = n;
+    }
     for (int i = 0; i < 4; ++i) lo.nb[i] = 0;
     lo.nblocks_site = 0;           // set by choose_site_tile()
     for (int i = 0; i < 4; ++i) lo.nbm[i] = 0;
@@ -360,7 +365,7 @@ struct Impl {
 #undef LGF_K1_CASE
         }
         CU(cudaGetLastError());
-        k1_finish<<<1, 256, 0, c->stream>>>(partials, nblocks, dev_state(c), (double)c->V, mode);
+        k1_finish<<<1, kFinishThreads, 0, c->stream>>>(partials, nblocks, dev_state(c), (double)c->V, mode);
         c->launches += 2;
         CU(cudaGetLastError());
         return LGF_OK;
@@ -377,7 +382,7 @@ struct Impl {
         void* args[] = {&u0, &u1, &dt, &dout, &partials, &st, &c->mgeom, &ha};
         const FusedEntry& e = fused_entries()[c->fused_tile];
         CU(cudaLaunchKernel(e.kernel, dim3(c->fused_grid), dim3(e.threads), args, e.smem, c->stream));
-        k1_finish<<<1, 256, 0, c->stream>>>(partials, c->fused_grid, dev_state(c), (double)c->V, 2);
+        k1_finish<<<1, kFinishThreads, 0, c->stream>>>(partials, c->fused_grid, dev_state(c), (double)c->V, 2);
         c->launches += 2;
         CU(cudaGetLastError());
         return LGF_OK;
@@ -438,10 +443,16 @@ struct Impl {
     }
     static int k5(lgf_ctx* c, double alpha) {
         if (c->site_variant == 2) {
+            // resident CTAs per SM the 256-thread k5s tiles are compiled for (LGF_K5S_OCC overrides at build time)
+#ifdef LGF_K5S_OCC
+            constexpr int kS3 = LGF_K5S_OCC;
+#else
+            constexpr int kS3 = sizeof(T) == 8 ? 3 : 4;
+#endif
 #define LGF_K5S_CASE(ID, TILE, MINB) case ID: k5s_gbuild_update<T, NC, TILE, MINB><<<c->nblocks_s, TILE::kThreads, 0, c->stream>>>( \
                 links(c), delta(c), dev_state(c), c->geom_s, (T)(0.5 * alpha)); break;
             switch (c->s_tile) {
-                LGF_K5S_CASE(1, TileS1, 1) LGF_K5S_CASE(2, TileS2, 2) LGF_K5S_CASE(3, TileS3, 2) LGF_K5S_CASE(4, TileS4, 1)
+                LGF_K5S_CASE(1, TileS1, 1) LGF_K5S_CASE(2, TileS2, kS3) LGF_K5S_CASE(3, TileS3, kS3) LGF_K5S_CASE(4, TileS4, 1)
                 default: k5s_gbuild_update<T, NC, TileS0, 2><<<c->nblocks_s, TileS0::kThreads, 0, c->stream>>>(
                     links(c), delta(c), dev_state(c), c->geom_s, (T)(0.5 * alpha));
             }
@@ -733,10 +744,9 @@ static int create_common(const int32_t L[4], int precision, int storage, void* w
     {   // K5 flavour: 0 = thread per (site, direction), 1 = thread per site (LGF_SITE_VARIANT / LGF_SITEMU_TILE: A/B knobs)
         const char* e = getenv("LGF_SITE_VARIANT");
         // measured at 32^4: the (site, direction) split wins for fp64 18-real and fp32 12-real
-        const bool mu_default = (precision == LGF_F64 && storage == LGF_REAL18) || (precision == LGF_F32 && storage == LGF_REAL12);
         // measured at 32^4: the shared-g (site, direction) kernel k5s wins for fp64 18-real (233 vs 247 us) and
         // fp32 12-real (102 vs 107 us); thread-per-site wins for fp64 12-real (175 vs 194 us) and fp32 18-real
-        c->site_variant = e ? atoi(e) : (mu_default ? 2 : 1);
+        c->site_variant = e ? atoi(e) : 2;
         int t = (L[0] % 16 == 0) ? 2 : 0;
         e = getenv("LGF_SITEMU_TILE");
         if (e && atoi(e) >= 0 && atoi(e) < kNumMuTiles) t = atoi(e);
@@ -764,6 +774,7 @@ static int create_common(const int32_t L[4], int precision, int storage, void* w
         }
         c->nblocks_s = n;
         if (c->site_variant == 2 && !ok) c->site_variant = mu_default_fallback;
+
     }
     int rc = LGF_OK;
     if (ws_bytes < c->lo.total || (reinterpret_cast<uintptr_t>(ws) % kAlign) != 0) rc = LGF_EINVAL;

@@ -33,7 +33,11 @@ struct DevState {
 // Resident CTAs per SM each site kernel is compiled for (= register cap 65536 / (256 * n)); measured
 // best of 1..4 per precision and storage at 32^4.
 template <typename T, int NC> struct SiteOcc {
+#ifdef LGF_K1_OCC
+    static constexpr int k1 = LGF_K1_OCC;
+#else
     static constexpr int k1 = sizeof(T) == 8 ? 2 : 3;
+#endif
     static constexpr int k5 = sizeof(T) == 8 ? 2 : (NC == 6 ? 4 : 2);
     static constexpr int k5m = sizeof(T) == 8 ? 2 : 3;
 };
@@ -122,29 +126,37 @@ k1_delta_theta_F(const Cx<T>* __restrict__ U, Cx<T>* __restrict__ D, double2* __
     double th = 0.0, fn = 0.0;
     if (valid) {
         const long long s = site_index(g, x);
-        Su3<T> M;
-#pragma unroll
-        for (int c = 0; c < 9; ++c) M.m[c] = Cx<T>(0, 0);
-        T retr = 0;
+        // only the anti-Hermitian traceless part of M = sum_mu [U_mu(x-mu) - U_mu(x)] is needed: accumulate its
+        // 9 reals link by link (the projection is linear) instead of the full 3x3 sum
+        Cx<T> c0(0, 0), c1(0, 0), c2(0, 0);
+        T a0 = 0, a1 = 0, a2 = 0, retr = 0;
         long long stride = 1;
 #pragma unroll
         for (int mu = 0; mu < 4; ++mu) {
             const long long sb = (x[mu] == 0) ? s + stride * (g.L[mu] - 1) : s - stride;
-            Su3<T> a, b;
             // measured at 32^4: evict-first link loads help K1 in fp32 (80 -> 69 us, the Delta it writes stays in
             // L2 for K2) and hurt in fp64 (122 -> 134 us, 18-real: the backward re-reads start missing L2)
-            load_link<T, NC, sizeof(T) == 4>(a, U, g.V, mu, s);
-            load_link<T, NC, sizeof(T) == 4>(b, U, g.V, mu, sb);
-#pragma unroll
-            for (int c = 0; c < 9; ++c) M.m[c] = M.m[c] + (b.m[c] - a.m[c]);
-            retr += a.m[0].re + a.m[4].re + a.m[8].re;
+            {
+                Su3<T> a;
+                load_link<T, NC, sizeof(T) == 4>(a, U, g.V, mu, s);
+                c0 = c0 - (a.m[1] - conj(a.m[3]));
+                c1 = c1 - (a.m[2] - conj(a.m[6]));
+                c2 = c2 - (a.m[5] - conj(a.m[7]));
+                a0 -= a.m[0].im; a1 -= a.m[4].im; a2 -= a.m[8].im;
+                retr += a.m[0].re + a.m[4].re + a.m[8].re;
+            }
+            {
+                Su3<T> b;
+                load_link<T, NC, sizeof(T) == 4>(b, U, g.V, mu, sb);
+                c0 = c0 + (b.m[1] - conj(b.m[3]));
+                c1 = c1 + (b.m[2] - conj(b.m[6]));
+                c2 = c2 + (b.m[5] - conj(b.m[7]));
+                a0 += b.m[0].im; a1 += b.m[4].im; a2 += b.m[8].im;
+            }
             stride *= g.L[mu];
         }
-        // A = M - M^+ : off-diagonals A01, A02, A12; diagonal i * 2 Im M_ii; remove trace/3
-        const Cx<T> c0 = M.m[1] - conj(M.m[3]);
-        const Cx<T> c1 = M.m[2] - conj(M.m[6]);
-        const Cx<T> c2 = M.m[5] - conj(M.m[7]);
-        const T a0 = T(2) * M.m[0].im, a1 = T(2) * M.m[4].im, a2 = T(2) * M.m[8].im;
+        // diagonal of A = M - M^+ is i * 2 Im M_ii; remove trace/3
+        a0 *= T(2); a1 *= T(2); a2 *= T(2);
         const T tr3 = (a0 + a1 + a2) / T(3);
         const T d0 = a0 - tr3, d1 = a1 - tr3, d2 = a2 - tr3;
         st_cx(D + s, c0);
@@ -164,16 +176,17 @@ k1_delta_theta_F(const Cx<T>* __restrict__ U, Cx<T>* __restrict__ D, double2* __
 // iteration count and evaluates the stopping test on the device (mode 2: end of a FUSED iteration,
 // which additionally swaps the roles of the two link buffers).  A separate tiny launch instead
 // of a last-CTA ticket: the K1 CTAs then retire without a fence + atomic tail.
-__global__ void __launch_bounds__(256)
+constexpr int kFinishThreads = 1024;
+__global__ void __launch_bounds__(kFinishThreads)
 k1_finish(const double2* __restrict__ partials, int n, DevState* st, double V, int mode) {
     if (mode >= 1 && *reinterpret_cast<volatile int*>(&st->done)) return;
     double a = 0.0, b = 0.0;
-    for (int i = threadIdx.x; i < n; i += 256) {
+    for (int i = threadIdx.x; i < n; i += kFinishThreads) {
         const double2 p = partials[i];
         a += p.x;
         b += p.y;
     }
-    block_sum2<256>(a, b);
+    block_sum2<kFinishThreads>(a, b);
     if (threadIdx.x == 0) {
         const double theta = a / (3.0 * V);
         st->theta = theta;
