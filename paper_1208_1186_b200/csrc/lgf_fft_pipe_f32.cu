@@ -28,6 +28,10 @@ const ZtPipeEntry* zt_pipe_table_f32(int* n) {
         ZtP<T, 32, 32, 32, 32, 4, 128, 2, 4>::entry(),
         ZtP<T, 32, 32, 32, 32, 8, 256, 2, 3>::entry(),
         ZtP<T, 48, 8, 8, 8, 8, 128, 3, 4>::entry(),
+        // the paper's other finite-temperature shapes 48^3 x N_t, N_t = 4, 6, 12
+        ZtP<T, 48, 8, 4, 4, 8, 128, 3, 4>::entry(),
+        ZtP<T, 48, 8, 6, 6, 8, 128, 3, 4>::entry(),
+        ZtP<T, 48, 8, 12, 12, 8, 128, 2, 3>::entry(),
         ZtP<T, 48, 8, 8, 8, 8, 256, 2, 4>::entry(),
         ZtPH<T, 64, 8, 64, 8, 4, 512>::entry(),
         ZtP<T, 64, 8, 64, 8, 4, 512, 1, 1>::entry(),

@@ -292,7 +292,8 @@ def test_fused_update_kernel(monkeypatch, L, prec, stor):
     gf.close()
 
 
-@pytest.mark.parametrize("L", [(8, 8, 64, 64), (64, 64, 8, 8), (48, 48, 8, 8), (8, 8, 48, 8)])
+@pytest.mark.parametrize("L", [(8, 8, 64, 64), (64, 64, 8, 8), (48, 48, 8, 8), (8, 8, 48, 8), (8, 8, 48, 4), (8, 8, 48, 6),
+                               (16, 16, 48, 12)])
 def test_large_extent_fft_kernels(L):
     """The 48- and 64-point two-stage line kernels (64^4's K3 runs on the half-tile ring) on lattices the
     oracle still finishes in seconds: two iterations in fp64 12-real and fp32 18-real."""
