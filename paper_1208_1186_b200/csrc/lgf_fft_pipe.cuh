@@ -202,10 +202,11 @@ fft_xy_pipe(const Cx<T>* in, Cx<T>* out, const XyPipeArgs A, const int* done) {
             group_sync<GT, NG>(g);
             // ---- coalesced copy-out, natural layout ----
             Cx<T>* base = out + (size_t)plane0 * PLANE;
+            const uint64_t keep = l2_evict_last_policy();      // Delta~ is K5's next read
 #pragma unroll 4
             for (int e = gtid; e < nvalid * PLANE; e += GT) {
                 const int x = e % NX, y = (e / NX) % NY, pl = e / PLANE;
-                st_cx(base + e, tile[pl * PLANE + y * NX + (x ^ (y & SW))]);
+                st_cx_keep(base + e, tile[pl * PLANE + y * NX + (x ^ (y & SW))], keep);
             }
         }
         // ---- hand the buffer back to the TMA unit for tile i + NBUF ----

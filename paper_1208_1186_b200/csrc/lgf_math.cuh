@@ -112,6 +112,24 @@ __device__ __forceinline__ void st_cx_stream(Cx<float>* p, Cx<float> a, uint64_t
 #endif
 }
 
+// Stores of a field the NEXT kernel reads in full and that fits the L2 (Delta out of K1, Delta~ out of K4):
+// evict-last, so that the links streaming through the same L2 do not push it out before it is consumed.
+#ifndef LGF_KEEP_DELTA
+#define LGF_KEEP_DELTA 1
+#endif
+__device__ __forceinline__ uint64_t l2_evict_last_policy() {
+    uint64_t p;
+    asm("createpolicy.fractional.L2::evict_last.b64 %0, 1.0;" : "=l"(p));
+    return p;
+}
+template <typename T> __device__ __forceinline__ void st_cx_keep(Cx<T>* p, Cx<T> a, uint64_t pol) {
+#if LGF_KEEP_DELTA
+    st_cx_stream(p, a, pol);      // same instruction, different policy operand
+#else
+    st_cx(p, a);
+#endif
+}
+
 // 3x3 complex matrix in registers, row-major m[3*row + col]
 template <typename T> struct Su3 { Cx<T> m[9]; };
 

@@ -159,10 +159,11 @@ k1_delta_theta_F(const Cx<T>* __restrict__ U, Cx<T>* __restrict__ D, double2* __
         a0 *= T(2); a1 *= T(2); a2 *= T(2);
         const T tr3 = (a0 + a1 + a2) / T(3);
         const T d0 = a0 - tr3, d1 = a1 - tr3, d2 = a2 - tr3;
-        st_cx(D + s, c0);
-        st_cx(D + (size_t)g.V + s, c1);
-        st_cx(D + (size_t)2 * g.V + s, c2);
-        st_cx(D + (size_t)3 * g.V + s, Cx<T>(d0, d1));
+        const uint64_t keep = l2_evict_last_policy();
+        st_cx_keep(D + s, c0, keep);
+        st_cx_keep(D + (size_t)g.V + s, c1, keep);
+        st_cx_keep(D + (size_t)2 * g.V + s, c2, keep);
+        st_cx_keep(D + (size_t)3 * g.V + s, Cx<T>(d0, d1), keep);
         th = 2.0 * ((double)norm2(c0) + (double)norm2(c1) + (double)norm2(c2)) + (double)d0 * d0 +
              (double)d1 * d1 + (double)d2 * d2;
         fn = (double)retr;
