@@ -64,9 +64,11 @@ typedef struct {
     int32_t converged;  /* theta < theta_tol (lgf_fix only; 0 otherwise) */
 } lgf_result;
 
-/* Bytes of device workspace lgf_create needs for this lattice (links in the device layout, the
- * packed Delta field (4 complex per site), reduction partials, twiddle and
- * p^2 tables, boundary staging).  Returns 0 if the arguments are invalid or unsupported. */
+/* Bytes of device workspace lgf_create needs for this lattice: two link buffers in the device
+ * layout (the fused update kernel writes out of place; the default path uses only the first), three
+ * packed Delta-sized fields (4 complex per site: Delta, the layout-B spectrum between
+ * K2 and K3, Delta~), reduction partials, twiddle and p^2 tables, boundary staging.  About
+ * (8 n_l + 24 (1 + 1/(3 Lz))) w bytes per site.  Returns 0 if the arguments are invalid or unsupported. */
 size_t lgf_workspace_bytes(const int32_t L[4], int precision, int storage);
 
 /* Create a context.  `workspace_dev` is DEVICE memory of at least lgf_workspace_bytes(...) bytes,
