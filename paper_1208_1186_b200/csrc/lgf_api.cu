@@ -167,6 +167,8 @@ struct lgf_ctx {
     ZtArgs zt_args;
     // pipelined fast path (lgf_fft_pipe.cuh); both set or both null
     const XyPipeEntry* xy_pipe;
+    const XyPipeEntry* xy_pipe_inv;      // K4's entry (same line splits as K2's, possibly another tile shape)
+    int xyp_inv_grid;
     const ZtPipeEntry* zt_pipe;
     XyPipeArgs xyp_args;
     int xyp_grid, ztp_grid;
@@ -276,6 +278,7 @@ bool plan_passes(lgf_ctx* c) {
     c->zt_pipe = find_zt_pipe(c->precision, L[2], L[3], LxLy);
     c->xy_pipe = c->zt_pipe ? find_xy_pipe(c->precision, L[0], L[1]) : nullptr;
     if (!c->xy_pipe) c->zt_pipe = nullptr;
+    c->xy_pipe_inv = c->xy_pipe ? find_xy_pipe_inv(c->precision, L[0], L[1], c->xy_pipe) : nullptr;
     {   // LGF_FFT_PIPE=0: fall back to the one-tile-per-CTA kernels (A/B knob)
         const char* e = getenv("LGF_FFT_PIPE");
         if (e && atoi(e) == 0) c->xy_pipe = nullptr, c->zt_pipe = nullptr;
@@ -497,11 +500,11 @@ struct Impl {
                 void* args[] = {&d2, &dptr, &c->zt_args, &done};          // layout B -> natural
                 CU(cudaLaunchKernel(e->kernel, dim3(c->ztp_grid), dim3(e->threads), args, e->smem, c->stream));
             } else {
-                const XyPipeEntry* e = c->xy_pipe;
+                const XyPipeEntry* e = k == 0 ? c->xy_pipe : c->xy_pipe_inv;
                 Cx<T>* inp = k == 0 ? delta_src(c) : dptr;                 // K2 reads Delta where K1 / K51 left it
                 Cx<T>* outp = k == 0 ? d2 : dptr;                          // K2: natural -> layout B; K4: in place
                 void* args[] = {&inp, &outp, &c->xyp_args, &done};
-                CU(cudaLaunchKernel(k == 0 ? e->k_fwd : e->k_inv, dim3(c->xyp_grid), dim3(e->threads), args, e->smem, c->stream));
+                CU(cudaLaunchKernel(k == 0 ? e->k_fwd : e->k_inv, dim3(k == 0 ? c->xyp_grid : c->xyp_inv_grid), dim3(e->threads), args, e->smem, c->stream));
             }
             c->launches++;
             return LGF_OK;
@@ -544,6 +547,10 @@ struct Impl {
             CU(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, c->xy_pipe->k_fwd, c->xy_pipe->threads, c->xy_pipe->smem));
             if (occ < 1) return cuda_fail(cudaErrorLaunchOutOfResources, "fft_xy_pipe does not fit on an SM");
             c->xyp_grid = xy_tiles < occ * sms ? xy_tiles : occ * sms;
+            const int inv_tiles = (c->xyp_args.nplanes + c->xy_pipe_inv->pb - 1) / c->xy_pipe_inv->pb;
+            CU(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, c->xy_pipe_inv->k_inv, c->xy_pipe_inv->threads, c->xy_pipe_inv->smem));
+            if (occ < 1) return cuda_fail(cudaErrorLaunchOutOfResources, "fft_xy_pipe (inverse) does not fit on an SM");
+            c->xyp_inv_grid = inv_tiles < occ * sms ? inv_tiles : occ * sms;
             const int zt_tiles = 4 * c->zt_args.tiles_per_comp;
             CU(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, c->zt_pipe->kernel, c->zt_pipe->threads, c->zt_pipe->smem));
             if (occ < 1) return cuda_fail(cudaErrorLaunchOutOfResources, "fft_zt_pipe does not fit on an SM");

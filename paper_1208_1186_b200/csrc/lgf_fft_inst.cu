@@ -61,6 +61,18 @@ cudaError_t prepare_ct_kernels(int precision) {
 static const XyPipeEntry* xyp_tab(int precision, int* n) { return precision ? xy_pipe_table_f64(n) : xy_pipe_table_f32(n); }
 static const ZtPipeEntry* ztp_tab(int precision, int* n) { return precision ? zt_pipe_table_f64(n) : zt_pipe_table_f32(n); }
 
+// K4 may run on a different tile shape than K2 (both read and write the natural layout on their own):
+// LGF_XYP_INV_VARIANT = v picks the v-th match; default -1 = "same entry as K2" unless a tuned default exists.
+const XyPipeEntry* find_xy_pipe_inv(int precision, int nx, int ny, const XyPipeEntry* fwd) {
+    const char* e = getenv("LGF_XYP_INV_VARIANT");
+    int skip = e ? atoi(e) : ((precision == 1 && nx == 32 && ny == 32 && !getenv("LGF_XYP_VARIANT")) ? 1 : -1);
+    if (skip < 0) return fwd;
+    int n = 0;
+    const XyPipeEntry* t = xyp_tab(precision, &n);
+    for (int i = 0; i < n; ++i)
+        if (t[i].nx == nx && t[i].ny == ny && t[i].x_n1 == fwd->x_n1 && t[i].y_n1 == fwd->y_n1 && skip-- == 0) return &t[i];
+    return fwd;
+}
 const XyPipeEntry* find_xy_pipe(int precision, int nx, int ny) {
     int n = 0, skip = variant("LGF_XYP_VARIANT");
     const XyPipeEntry* t = xyp_tab(precision, &n);

@@ -29,6 +29,7 @@ struct ZtPipeEntry {
 
 // precision: 0 = float, 1 = double; LGF_XYP_VARIANT / LGF_ZTP_VARIANT pick the v-th match (A/B knob)
 const XyPipeEntry* find_xy_pipe(int precision, int nx, int ny);
+const XyPipeEntry* find_xy_pipe_inv(int precision, int nx, int ny, const XyPipeEntry* fwd);
 const ZtPipeEntry* find_zt_pipe(int precision, int nz, int nt, long long LxLy);
 cudaError_t prepare_pipe_kernels(int precision);
 
