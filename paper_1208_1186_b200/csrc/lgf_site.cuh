@@ -46,8 +46,11 @@ template <int TX, int TY, int TZ, int TT>
 struct SiteTile {
     static constexpr int kThreads = TX * TY * TZ * TT;
     // thread -> lattice coordinates of its site; returns false outside the lattice
+    // REVERSE: walk the tiles from the last to the first.  K1 does (it follows K5, which walks forward, so the
+    // links K5 wrote last are still in L2 when K1 starts with them).
+    template <bool REVERSE = false>
     __device__ static __forceinline__ bool coords(const Geom& g, int x[4]) {
-        int b = blockIdx.x;
+        int b = REVERSE ? (int)(gridDim.x - 1 - blockIdx.x) : (int)blockIdx.x;
         const int bx = b % g.nb[0]; b /= g.nb[0];
         const int by = b % g.nb[1]; b /= g.nb[1];
         const int bz = b % g.nb[2]; b /= g.nb[2];
@@ -122,7 +125,11 @@ k1_delta_theta_F(const Cx<T>* __restrict__ U, Cx<T>* __restrict__ D, double2* __
                  const DevState* st, Geom g, int mode) {
     if (mode == 1 && *reinterpret_cast<const volatile int*>(&st->done)) return;
     int x[4];
-    const bool valid = Tile::coords(g, x);
+#ifndef LGF_K1_FORWARD
+    const bool valid = Tile::template coords<true>(g, x);
+#else
+    const bool valid = Tile::template coords<false>(g, x);
+#endif
     double th = 0.0, fn = 0.0;
     if (valid) {
         const long long s = site_index(g, x);
