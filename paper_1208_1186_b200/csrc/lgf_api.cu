@@ -188,9 +188,44 @@ struct lgf_ctx {
     DevState* host_state;
     cudaEvent_t ev[2];
     int64_t pending_n;           // lgf_iterate_async bookkeeping (-1: nothing pending)
+    // programmatic dependent launch: set while the iteration body is captured, so that every kernel after the
+    // first becomes a programmatic edge of the graph (its CTAs are scheduled while the previous kernel drains
+    // and block in griddepcontrol.wait, see pdl_entry()); LGF_PDL=0 turns it off
+    bool pdl_enabled, pdl;
+    int pdl_mask, pdl_idx;       // which launches of the body (bit i: i-th launch) carry the attribute
 };
 
 namespace {
+
+// kernel launches of the iteration body (typed, and through the instantiation tables' untyped pointers)
+cudaLaunchConfig_t launch_config(lgf_ctx* c, dim3 grid, dim3 block, size_t smem, cudaLaunchAttribute* at) {
+    cudaLaunchConfig_t cfg = {};
+    cfg.gridDim = grid;
+    cfg.blockDim = block;
+    cfg.dynamicSmemBytes = smem;
+    cfg.stream = c->stream;
+    at->id = cudaLaunchAttributeProgrammaticStreamSerialization;
+    at->val.programmaticStreamSerializationAllowed = 1;
+    cfg.attrs = at;
+    cfg.numAttrs = (c->pdl && ((c->pdl_mask >> c->pdl_idx) & 1)) ? 1 : 0;
+    c->pdl_idx++;
+    return cfg;
+}
+template <typename... KArgs, typename... Args>
+cudaError_t launch_ex(lgf_ctx* c, void (*kernel)(KArgs...), dim3 grid, dim3 block, size_t smem, Args&&... args) {
+    cudaLaunchAttribute at;
+    const cudaLaunchConfig_t cfg = launch_config(c, grid, block, smem, &at);
+    return cudaLaunchKernelEx(&cfg, kernel, KArgs(args)...);
+}
+cudaError_t launch_exc(lgf_ctx* c, const void* kernel, dim3 grid, dim3 block, void** args, size_t smem) {
+    cudaLaunchAttribute at;
+    const cudaLaunchConfig_t cfg = launch_config(c, grid, block, smem, &at);
+    return cudaLaunchKernelExC(&cfg, kernel, args);
+}
+
+// grid of the site kernels: (x tiles, y tiles, z tiles * t tiles); see split_zt()
+dim3 grid3(const Geom& g) { return dim3((unsigned)g.nb[0], (unsigned)g.nb[1], (unsigned)(g.nb[2] * g.nb[3])); }
+void set_magic(Geom& g) { g.nb2_magic = g.nb[2] > 1 ? (unsigned)((0x100000000ULL + (unsigned)g.nb[2] - 1) / (unsigned)g.nb[2]) : 0u; }
 
 DevState* dev_state(lgf_ctx* c) { return reinterpret_cast<DevState*>(c->ws + c->lo.state); }
 
@@ -358,17 +393,17 @@ struct Impl {
         int nblocks;
         {
             nblocks = c->lo.nblocks_site;
-#define LGF_K1_CASE(ID, TILE) case ID: k1_delta_theta_F<T, NC, TILE><<<nblocks, TILE::kThreads, 0, c->stream>>>( \
+#define LGF_K1_CASE(ID, TILE) case ID: launch_ex(c, k1_delta_theta_F<T, NC, TILE>, grid3(c->geom), dim3(TILE::kThreads), 0,  \
                 links(c), delta_src(c), partials, dev_state(c), c->geom, mode); break;
             switch (c->site_tile) {
                 LGF_K1_CASE(1, Tile1) LGF_K1_CASE(2, Tile2) LGF_K1_CASE(3, Tile3) LGF_K1_CASE(4, Tile4) LGF_K1_CASE(5, Tile5)
-                default: k1_delta_theta_F<T, NC, Tile0><<<nblocks, Tile0::kThreads, 0, c->stream>>>(
+                default: launch_ex(c, k1_delta_theta_F<T, NC, Tile0>, grid3(c->geom), dim3(Tile0::kThreads), 0, 
                     links(c), delta_src(c), partials, dev_state(c), c->geom, mode);
             }
 #undef LGF_K1_CASE
         }
         CU(cudaGetLastError());
-        k1_finish<<<1, kFinishThreads, 0, c->stream>>>(partials, nblocks, dev_state(c), (double)c->V, mode);
+        launch_ex(c, k1_finish, dim3(1), dim3(kFinishThreads), 0, partials, nblocks, dev_state(c), (double)c->V, mode);
         c->launches += 2;
         CU(cudaGetLastError());
         return LGF_OK;
@@ -384,8 +419,8 @@ struct Impl {
         T ha = (T)(0.5 * alpha);
         void* args[] = {&u0, &u1, &dt, &dout, &partials, &st, &c->mgeom, &ha};
         const FusedEntry& e = fused_entries()[c->fused_tile];
-        CU(cudaLaunchKernel(e.kernel, dim3(c->fused_grid), dim3(e.threads), args, e.smem, c->stream));
-        k1_finish<<<1, kFinishThreads, 0, c->stream>>>(partials, c->fused_grid, dev_state(c), (double)c->V, 2);
+        CU(launch_exc(c, e.kernel, dim3(c->fused_grid), dim3(e.threads), args, e.smem));
+        launch_ex(c, k1_finish, dim3(1), dim3(kFinishThreads), 0, partials, c->fused_grid, dev_state(c), (double)c->V, 2);
         c->launches += 2;
         CU(cudaGetLastError());
         return LGF_OK;
@@ -452,11 +487,11 @@ struct Impl {
 #else
             constexpr int kS3 = sizeof(T) == 8 ? 3 : 4;
 #endif
-#define LGF_K5S_CASE(ID, TILE, MINB) case ID: k5s_gbuild_update<T, NC, TILE, MINB><<<c->nblocks_s, TILE::kThreads, 0, c->stream>>>( \
+#define LGF_K5S_CASE(ID, TILE, MINB) case ID: launch_ex(c, k5s_gbuild_update<T, NC, TILE, MINB>, grid3(c->geom_s), dim3(TILE::kThreads), 0,  \
                 links(c), delta(c), dev_state(c), c->geom_s, (T)(0.5 * alpha)); break;
             switch (c->s_tile) {
                 LGF_K5S_CASE(1, TileS1, 1) LGF_K5S_CASE(2, TileS2, kS3) LGF_K5S_CASE(3, TileS3, kS3) LGF_K5S_CASE(4, TileS4, 1)
-                default: k5s_gbuild_update<T, NC, TileS0, 2><<<c->nblocks_s, TileS0::kThreads, 0, c->stream>>>(
+                default: launch_ex(c, k5s_gbuild_update<T, NC, TileS0, 2>, grid3(c->geom_s), dim3(TileS0::kThreads), 0, 
                     links(c), delta(c), dev_state(c), c->geom_s, (T)(0.5 * alpha));
             }
 #undef LGF_K5S_CASE
@@ -465,11 +500,11 @@ struct Impl {
             return LGF_OK;
         }
         if (c->site_variant == 0) {
-#define LGF_K5M_CASE(ID, TILE) case ID: k5m_gbuild_update<T, NC, TILE><<<c->lo.nblocks_mu, TILE::kThreads, 0, c->stream>>>( \
+#define LGF_K5M_CASE(ID, TILE) case ID: launch_ex(c, k5m_gbuild_update<T, NC, TILE>, grid3(c->geom_mu), dim3(TILE::kThreads), 0,  \
                 links(c), delta(c), dev_state(c), c->geom_mu, (T)(0.5 * alpha)); break;
             switch (c->mu_tile) {
                 LGF_K5M_CASE(1, TileM1) LGF_K5M_CASE(2, TileM2)
-                default: k5m_gbuild_update<T, NC, TileM0><<<c->lo.nblocks_mu, TileM0::kThreads, 0, c->stream>>>(
+                default: launch_ex(c, k5m_gbuild_update<T, NC, TileM0>, grid3(c->geom_mu), dim3(TileM0::kThreads), 0, 
                     links(c), delta(c), dev_state(c), c->geom_mu, (T)(0.5 * alpha));
             }
 #undef LGF_K5M_CASE
@@ -477,11 +512,11 @@ struct Impl {
             CU(cudaGetLastError());
             return LGF_OK;
         }
-#define LGF_K5_CASE(ID, TILE) case ID: k5_gbuild_update<T, NC, TILE><<<c->lo.nblocks_site, TILE::kThreads, 0, c->stream>>>( \
+#define LGF_K5_CASE(ID, TILE) case ID: launch_ex(c, k5_gbuild_update<T, NC, TILE>, grid3(c->geom), dim3(TILE::kThreads), 0,  \
             links(c), delta(c), dev_state(c), c->geom, (T)(0.5 * alpha)); break;
         switch (c->site_tile) {
             LGF_K5_CASE(1, Tile1) LGF_K5_CASE(2, Tile2) LGF_K5_CASE(3, Tile3) LGF_K5_CASE(4, Tile4) LGF_K5_CASE(5, Tile5)
-            default: k5_gbuild_update<T, NC, Tile0><<<c->lo.nblocks_site, Tile0::kThreads, 0, c->stream>>>(
+            default: launch_ex(c, k5_gbuild_update<T, NC, Tile0>, grid3(c->geom), dim3(Tile0::kThreads), 0, 
                 links(c), delta(c), dev_state(c), c->geom, (T)(0.5 * alpha));
         }
 #undef LGF_K5_CASE
@@ -498,13 +533,13 @@ struct Impl {
             if (k == 1) {
                 const ZtPipeEntry* e = c->zt_pipe;
                 void* args[] = {&d2, &dptr, &c->zt_args, &done};          // layout B -> natural
-                CU(cudaLaunchKernel(e->kernel, dim3(c->ztp_grid), dim3(e->threads), args, e->smem, c->stream));
+                CU(launch_exc(c, e->kernel, dim3(c->ztp_grid), dim3(e->threads), args, e->smem));
             } else {
                 const XyPipeEntry* e = k == 0 ? c->xy_pipe : c->xy_pipe_inv;
                 Cx<T>* inp = k == 0 ? delta_src(c) : dptr;                 // K2 reads Delta where K1 / K51 left it
                 Cx<T>* outp = k == 0 ? d2 : dptr;                          // K2: natural -> layout B; K4: in place
                 void* args[] = {&inp, &outp, &c->xyp_args, &done};
-                CU(cudaLaunchKernel(k == 0 ? e->k_fwd : e->k_inv, dim3(k == 0 ? c->xyp_grid : c->xyp_inv_grid), dim3(e->threads), args, e->smem, c->stream));
+                CU(launch_exc(c, k == 0 ? e->k_fwd : e->k_inv, dim3(k == 0 ? c->xyp_grid : c->xyp_inv_grid), dim3(e->threads), args, e->smem));
             }
             c->launches++;
             return LGF_OK;
@@ -512,23 +547,23 @@ struct Impl {
         if (k != 1 && c->xy_ct) {
             const XyCtEntry* e = c->xy_ct;
             void* args[] = {&dptr, &c->xy_args, &done};
-            CU(cudaLaunchKernel(k == 0 ? e->k_fwd : e->k_inv, dim3((planes + e->pb - 1) / e->pb), dim3(e->threads), args, e->smem, c->stream));
+            CU(launch_exc(c, k == 0 ? e->k_fwd : e->k_inv, dim3((planes + e->pb - 1) / e->pb), dim3(e->threads), args, e->smem));
             c->launches++;
             return LGF_OK;
         }
         if (k == 1 && c->zt_ct) {
             const ZtCtEntry* e = c->zt_ct;
             void* args[] = {&dptr, &c->zt_args, &done};
-            CU(cudaLaunchKernel(e->kernel, dim3(4 * c->zt_args.tiles_per_comp), dim3(e->threads), args, e->smem, c->stream));
+            CU(launch_exc(c, e->kernel, dim3(4 * c->zt_args.tiles_per_comp), dim3(e->threads), args, e->smem));
             c->launches++;
             return LGF_OK;
         }
         if (k == 0)
-            fft_xy_kernel<T, -1><<<planes, c->xy_threads, c->xy_smem, c->stream>>>(delta(c), c->xy, done);
+            launch_ex(c, fft_xy_kernel<T, -1>, dim3(planes), dim3(c->xy_threads), c->xy_smem, delta(c), c->xy, done);
         else if (k == 2)
-            fft_xy_kernel<T, +1><<<planes, c->xy_threads, c->xy_smem, c->stream>>>(delta(c), c->xy, done);
+            launch_ex(c, fft_xy_kernel<T, +1>, dim3(planes), dim3(c->xy_threads), c->xy_smem, delta(c), c->xy, done);
         else
-            fft_zt_kernel<T><<<4 * c->zt.tiles_per_comp, c->zt_threads, c->zt_smem, c->stream>>>(delta(c), c->zt, c->V, done);
+            launch_ex(c, fft_zt_kernel<T>, dim3(4 * c->zt.tiles_per_comp), dim3(c->zt_threads), c->zt_smem, delta(c), c->zt, c->V, done);
         c->launches++;
         CU(cudaGetLastError());
         return LGF_OK;
@@ -643,7 +678,11 @@ struct Impl {
 
 int enqueue_iteration_body(lgf_ctx* c, double alpha) {
     int rc;
+    c->pdl = false;                 // the first kernel of the graph has no predecessor to overlap with
+    c->pdl_idx = 0;
     if ((rc = DISPATCH(c, fft(c, 0, true)))) return rc;
+    cudaStreamCaptureStatus cs = cudaStreamCaptureStatusNone;
+    if (cudaStreamIsCapturing(c->stream, &cs) == cudaSuccess && cs == cudaStreamCaptureStatusActive) c->pdl = c->pdl_enabled;
     if ((rc = DISPATCH(c, fft(c, 1, true)))) return rc;
     if ((rc = DISPATCH(c, fft(c, 2, true)))) return rc;
     if (c->fused_tile >= 0) return DISPATCH(c, k51(c, alpha));
@@ -662,6 +701,7 @@ int ensure_graph(lgf_ctx* c, double alpha) {
     c->stream = c->cap_stream;
     const int rc = enqueue_iteration_body(c, alpha);
     c->stream = user;
+    c->pdl = false;
     cudaGraph_t g = nullptr;
     cudaError_t e = cudaStreamEndCapture(c->cap_stream, &g);
     c->launches_per_iter = (int)(c->launches - before);
@@ -737,6 +777,14 @@ static int create_common(const int32_t L[4], int precision, int storage, void* w
     c->stream = reinterpret_cast<cudaStream_t>(stream);
     c->lo = make_layout(L, precision, storage);
     c->pending_n = -1;
+    {
+        const char* e = getenv("LGF_PDL");
+        // measured: 8^4 22.6 -> 20.5 us per iteration, 16^4 32.8 -> 32.0 us, but 32^4 fp64-12 315 -> 381 us
+        // with every edge programmatic (no single edge gains more than 1.5 us there), so: launch-bound lattices only
+        c->pdl_enabled = e ? atoi(e) != 0 : c->V <= 65536;
+        e = getenv("LGF_PDL_MASK");
+        c->pdl_mask = e ? atoi(e) : 0x3e;
+    }
     {   // thread-per-site tiling: widest x tile that divides Lx (LGF_SITE_TILE overrides, A/B knob)
         int t = (L[0] % 32 == 0) ? 4 : ((L[0] % 16 == 0) ? 1 : 0);
         const char* e = getenv("LGF_SITE_TILE");
@@ -747,6 +795,7 @@ static int create_common(const int32_t L[4], int precision, int storage, void* w
         c->lo.nblocks_site = n;
     }
     for (int i = 0; i < 4; ++i) { c->geom.L[i] = L[i]; c->geom.nb[i] = c->lo.nb[i]; }
+    set_magic(c->geom);
     c->geom.V = c->V;
     {   // K5 flavour: 0 = thread per (site, direction), 1 = thread per site (LGF_SITE_VARIANT / LGF_SITEMU_TILE: A/B knobs)
         const char* e = getenv("LGF_SITE_VARIANT");
@@ -764,6 +813,7 @@ static int create_common(const int32_t L[4], int precision, int storage, void* w
     }
     c->geom_mu = c->geom;
     for (int i = 0; i < 4; ++i) c->geom_mu.nb[i] = c->lo.nbm[i];
+    set_magic(c->geom_mu);
     const int mu_default_fallback = ((precision == LGF_F64 && storage == LGF_REAL18) || (precision == LGF_F32 && storage == LGF_REAL12)) ? 0 : 1;
     {   // shared-g K5 (LGF_SITE_VARIANT=2, LGF_SITES_TILE): needs every extent to be a multiple of the tile's
         const char* e = getenv("LGF_SITES_TILE");
@@ -780,6 +830,7 @@ static int create_common(const int32_t L[4], int precision, int storage, void* w
             n *= c->geom_s.nb[i] > 0 ? c->geom_s.nb[i] : 1;
         }
         c->nblocks_s = n;
+        set_magic(c->geom_s);
         if (c->site_variant == 2 && !ok) c->site_variant = mu_default_fallback;
 
     }

@@ -168,6 +168,7 @@ template <typename T> struct FftBounds { static constexpr int kMaxThreads = size
 template <typename T, int SIGN>
 __global__ void __launch_bounds__(FftBounds<T>::kMaxThreads, 1)
 fft_xy_kernel(Cx<T>* __restrict__ D, const XyPass P, const int* done) {
+    pdl_entry();
     extern __shared__ __align__(16) unsigned char smem_raw[];
     if (done && *reinterpret_cast<const volatile int*>(done)) return;
     Cx<T>* tile = reinterpret_cast<Cx<T>*>(smem_raw);
@@ -196,6 +197,7 @@ fft_xy_kernel(Cx<T>* __restrict__ D, const XyPass P, const int* done) {
 template <typename T>
 __global__ void __launch_bounds__(FftBounds<T>::kMaxThreads, 1)
 fft_zt_kernel(Cx<T>* __restrict__ D, const ZtPass P, long long V, const int* done) {
+    pdl_entry();
     extern __shared__ __align__(16) unsigned char smem_raw[];
     if (done && *reinterpret_cast<const volatile int*>(done)) return;
     Cx<T>* tile = reinterpret_cast<Cx<T>*>(smem_raw);

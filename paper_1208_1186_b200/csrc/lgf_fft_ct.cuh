@@ -78,6 +78,7 @@ struct XyArgs {
 template <typename T, class SX, class SY, int SIGN, int PB, int NTHREADS, int MINB>
 __global__ void __launch_bounds__(NTHREADS, MINB)
 fft_xy_ct(Cx<T>* __restrict__ D, const XyArgs A, const int* done) {
+    pdl_entry();
     extern __shared__ __align__(16) unsigned char smem_raw[];
     if (done && *reinterpret_cast<const volatile int*>(done)) return;
     constexpr int NX = SX::kN, NY = SY::kN, PX = NX + 1, PLANE = PX * NY;
@@ -204,6 +205,7 @@ struct ZtArgs {
 template <typename T, class SZ, class ST_, int CX, int NTHREADS, int MINB>
 __global__ void __launch_bounds__(NTHREADS, MINB)
 fft_zt_ct(Cx<T>* __restrict__ D, const ZtArgs A, const int* done) {
+    pdl_entry();
     extern __shared__ __align__(16) unsigned char smem_raw[];
     if (done && *reinterpret_cast<const volatile int*>(done)) return;
     constexpr int NZ = SZ::kN, NT = ST_::kN, PZ = CX, PT = CX * (NZ + 1);

@@ -68,6 +68,7 @@ template <typename T, int NX> struct XySwz {
 template <typename T, class SX, class SY, int SIGN, int PB, int GT, int NG, int NBUF>
 __global__ void __launch_bounds__(GT * NG, 1)
 fft_xy_pipe(const Cx<T>* in, Cx<T>* out, const XyPipeArgs A, const int* done) {
+    pdl_entry();
     extern __shared__ __align__(128) unsigned char pipe_smem[];
     if (done && *reinterpret_cast<const volatile int*>(done)) return;
     constexpr int NX = SX::kN, NY = SY::kN, PLANE = NX * NY, TILE = PB * PLANE, SW = XySwz<T, NX>::mask;
@@ -221,6 +222,7 @@ fft_xy_pipe(const Cx<T>* in, Cx<T>* out, const XyPipeArgs A, const int* done) {
 template <typename T, class SZ, class ST_, int CX, int GT, int NG, int NBUF>
 __global__ void __launch_bounds__(GT * NG, 1)
 fft_zt_pipe(const Cx<T>* inB, Cx<T>* out, const ZtArgs A, const int* done) {
+    pdl_entry();
     extern __shared__ __align__(128) unsigned char pipe_smem[];
     if (done && *reinterpret_cast<const volatile int*>(done)) return;
     constexpr int NZ = SZ::kN, NT = ST_::kN, PZ = CX, PT = CX * (NZ + 1), TILE = PT * NT;
@@ -366,6 +368,7 @@ fft_zt_pipe(const Cx<T>* inB, Cx<T>* out, const ZtArgs A, const int* done) {
 template <typename T, class SZ, class ST_, int CX, int GT>
 __global__ void __launch_bounds__(GT, 1)
 fft_zt_pipe_halves(const Cx<T>* inB, Cx<T>* out, const ZtArgs A, const int* done) {
+    pdl_entry();
     extern __shared__ __align__(128) unsigned char pipe_smem[];
     if (done && *reinterpret_cast<const volatile int*>(done)) return;
     constexpr int NZ = SZ::kN, NT = ST_::kN, PZ = CX, PT = CX * (NZ + 1), HT = NT / 2, HALF = PT * HT;

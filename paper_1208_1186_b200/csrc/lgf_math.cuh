@@ -48,7 +48,12 @@ template <typename T> __device__ __forceinline__ T norm2(Cx<T> a) { return a.re 
 template <typename T> __device__ __forceinline__ Cx<T> mul_i(Cx<T> a) { return Cx<T>(-a.im, a.re); }
 template <typename T> __device__ __forceinline__ Cx<T> mul_mi(Cx<T> a) { return Cx<T>(a.im, -a.re); }
 
-__device__ __forceinline__ float rsqrt_t(float x) { return 1.0f / sqrtf(x); }
+// fp32: MUFU.RSQ + one Newton step (~1 ulp) instead of sqrt and divide with their slow-path branches (~25 instructions
+// each, 7 per site in K5, which is issue-bound in fp32); fp64 keeps the correctly rounded 1/sqrt.
+__device__ __forceinline__ float rsqrt_t(float x) {
+    const float y = rsqrtf(x);
+    return y * fmaf(-0.5f * x * y, y, 1.5f);
+}
 __device__ __forceinline__ double rsqrt_t(double x) { return 1.0 / sqrt(x); }
 
 // Streaming 16-byte / 8-byte global accesses of one complex number.
@@ -109,6 +114,18 @@ __device__ __forceinline__ void st_cx_stream(Cx<float>* p, Cx<float> a, uint64_t
     asm volatile("st.global.L2::cache_hint.v2.f32 [%0], {%1, %2}, %3;" ::"l"(p), "f"(a.re), "f"(a.im), "l"(pol) : "memory");
 #else
     st_cx(p, a);
+#endif
+}
+
+// Programmatic dependent launch (sm_90+), first statement of every kernel of the iteration: wait until the kernel
+// this one depends on has completed and its writes are visible, then let the NEXT kernel of the chain be
+// scheduled as soon as every CTA of this one has started (its CTAs fill SMs as ours retire and block in their
+// own wait).  Every kernel of the chain waits, so completion is transitive.  Both instructions are no-ops
+// when the launch carries no programmatic dependency.
+__device__ __forceinline__ void pdl_entry() {
+    asm volatile("griddepcontrol.wait;" ::: "memory");
+#ifndef LGF_PDL_NOTRIGGER
+    asm volatile("griddepcontrol.launch_dependents;" ::: "memory");
 #endif
 }
 

@@ -13,9 +13,19 @@ namespace lgf {
 
 struct Geom {
     int L[4];    // Lx, Ly, Lz, Lt
-    int nb[4];   // tiles per axis for the per-site kernels
+    int nb[4];   // tiles per axis for the per-site kernels; launched as a (nb0, nb1, nb2 * nb3) grid
     long long V;
+    unsigned int nb2_magic;   // ceil(2^32 / nb2): blockIdx.z / nb2 by one multiply (see split_zt)
 };
+
+// The site kernels are launched on a 3-D grid (x tiles, y tiles, z tiles * t tiles): same CTA order as a linear
+// grid, but no runtime integer divisions in the prologue (they were ~100 of k5s's ~600 instructions per thread
+// and sat in front of the first load).  bzt < 2^16 and nb2 < 2^16, so the multiply-high quotient is exact.
+__device__ __forceinline__ void split_zt(const Geom& g, unsigned bzt, unsigned& bz, unsigned& bt) {
+    bt = g.nb[2] == 1 ? bzt : __umulhi(bzt, g.nb2_magic);
+    bz = bzt - bt * (unsigned)g.nb[2];
+}
+__device__ __forceinline__ unsigned linear_block() { return blockIdx.x + gridDim.x * (blockIdx.y + gridDim.y * blockIdx.z); }
 
 // Loop / reduction state, lives in the workspace (device memory).
 struct DevState {
@@ -50,11 +60,10 @@ struct SiteTile {
     // links K5 wrote last are still in L2 when K1 starts with them).
     template <bool REVERSE = false>
     __device__ static __forceinline__ bool coords(const Geom& g, int x[4]) {
-        int b = REVERSE ? (int)(gridDim.x - 1 - blockIdx.x) : (int)blockIdx.x;
-        const int bx = b % g.nb[0]; b /= g.nb[0];
-        const int by = b % g.nb[1]; b /= g.nb[1];
-        const int bz = b % g.nb[2]; b /= g.nb[2];
-        const int bt = b;
+        const unsigned bx = REVERSE ? gridDim.x - 1 - blockIdx.x : blockIdx.x;
+        const unsigned by = REVERSE ? gridDim.y - 1 - blockIdx.y : blockIdx.y;
+        unsigned bz, bt;
+        split_zt(g, REVERSE ? gridDim.z - 1 - blockIdx.z : blockIdx.z, bz, bt);
         int t = threadIdx.x;
         x[0] = bx * TX + t % TX; t /= TX;
         x[1] = by * TY + t % TY; t /= TY;
@@ -64,8 +73,9 @@ struct SiteTile {
     }
 };
 
+// (32-bit arithmetic: V < 2^31, a lattice beyond that would need > 1 TB of links)
 __device__ __forceinline__ long long site_index(const Geom& g, const int x[4]) {
-    return x[0] + (long long)g.L[0] * (x[1] + (long long)g.L[1] * (x[2] + (long long)g.L[2] * x[3]));
+    return (long long)(x[0] + g.L[0] * (x[1] + g.L[1] * (x[2] + g.L[2] * x[3])));
 }
 __device__ __forceinline__ long long axis_stride(const Geom& g, int mu) {
     long long s = 1;
@@ -123,6 +133,7 @@ template <typename T, int NC, class Tile>
 __global__ void __launch_bounds__(Tile::kThreads, SiteOcc<T, NC>::k1)
 k1_delta_theta_F(const Cx<T>* __restrict__ U, Cx<T>* __restrict__ D, double2* __restrict__ partials,
                  const DevState* st, Geom g, int mode) {
+    pdl_entry();
     if (mode == 1 && *reinterpret_cast<const volatile int*>(&st->done)) return;
     int x[4];
 #ifndef LGF_K1_FORWARD
@@ -132,15 +143,15 @@ k1_delta_theta_F(const Cx<T>* __restrict__ U, Cx<T>* __restrict__ D, double2* __
 #endif
     double th = 0.0, fn = 0.0;
     if (valid) {
-        const long long s = site_index(g, x);
+        const int s = (int)site_index(g, x);
         // only the anti-Hermitian traceless part of M = sum_mu [U_mu(x-mu) - U_mu(x)] is needed: accumulate its
         // 9 reals link by link (the projection is linear) instead of the full 3x3 sum
         Cx<T> c0(0, 0), c1(0, 0), c2(0, 0);
         T a0 = 0, a1 = 0, a2 = 0, retr = 0;
-        long long stride = 1;
+        int stride = 1;
 #pragma unroll
         for (int mu = 0; mu < 4; ++mu) {
-            const long long sb = (x[mu] == 0) ? s + stride * (g.L[mu] - 1) : s - stride;
+            const int sb = (x[mu] == 0) ? s + stride * (g.L[mu] - 1) : s - stride;
             // measured at 32^4: evict-first link loads help K1 in fp32 (80 -> 69 us, the Delta it writes stays in
             // L2 for K2) and hurt in fp64 (122 -> 134 us, 18-real: the backward re-reads start missing L2)
             {
@@ -176,7 +187,7 @@ k1_delta_theta_F(const Cx<T>* __restrict__ U, Cx<T>* __restrict__ D, double2* __
         fn = (double)retr;
     }
     block_sum2<Tile::kThreads>(th, fn);
-    if (threadIdx.x == 0) partials[blockIdx.x] = make_double2(th, fn);   // summed by k1_finish
+    if (threadIdx.x == 0) partials[linear_block()] = make_double2(th, fn);   // summed by k1_finish
 }
 
 // Second half of K1: one CTA sums the per-CTA (theta, F) partials in index order (deterministic, no
@@ -187,6 +198,7 @@ k1_delta_theta_F(const Cx<T>* __restrict__ U, Cx<T>* __restrict__ D, double2* __
 constexpr int kFinishThreads = 1024;
 __global__ void __launch_bounds__(kFinishThreads)
 k1_finish(const double2* __restrict__ partials, int n, DevState* st, double V, int mode) {
+    pdl_entry();
     if (mode >= 1 && *reinterpret_cast<volatile int*>(&st->done)) return;
     double a = 0.0, b = 0.0;
     for (int i = threadIdx.x; i < n; i += kFinishThreads) {
@@ -223,6 +235,7 @@ __device__ __forceinline__ void load_g(Su3<T>& g, const Cx<T>* __restrict__ D, l
 template <typename T, int NC, class Tile>
 __global__ void __launch_bounds__(Tile::kThreads, SiteOcc<T, NC>::k5)
 k5_gbuild_update(Cx<T>* __restrict__ U, const Cx<T>* __restrict__ D, const DevState* st, Geom g, T half_alpha) {
+    pdl_entry();
     if (*reinterpret_cast<const volatile int*>(&st->done)) return;
     int x[4];
     if (!Tile::coords(g, x)) return;

@@ -125,6 +125,7 @@ template <typename T, int NC, class Tile, int MINB>
 __global__ void __launch_bounds__(Tile::NS, MINB)
 k51_update_delta(const Cx<T>* __restrict__ U0, const Cx<T>* __restrict__ U1, const Cx<T>* __restrict__ Dt,
                  Cx<T>* __restrict__ Dout, double2* __restrict__ partials, const DevState* st, MarchGeom g, T ha) {
+    pdl_entry();
     extern __shared__ __align__(16) unsigned char fused_smem[];
     if (*reinterpret_cast<const volatile int*>(&st->done)) return;
     constexpr int TX = Tile::TX, TY = Tile::TY, TZ = Tile::TZ, NS = Tile::NS, NG = Tile::NG, NH = Tile::NH, NR = NC / 3;

@@ -17,11 +17,9 @@ struct SiteTileMu {
     static_assert(kSites % 32 == 0, "mu must be warp-uniform");
     static constexpr int tx = TX, ty = TY, tz = TZ, tt = TT;
     __device__ static __forceinline__ bool coords(const Geom& g, int ls, int x[4]) {
-        int b = blockIdx.x;
-        const int bx = b % g.nb[0]; b /= g.nb[0];
-        const int by = b % g.nb[1]; b /= g.nb[1];
-        const int bz = b % g.nb[2]; b /= g.nb[2];
-        const int bt = b;
+        const unsigned bx = blockIdx.x, by = blockIdx.y;
+        unsigned bz, bt;
+        split_zt(g, blockIdx.z, bz, bt);
         x[0] = bx * TX + ls % TX; ls /= TX;
         x[1] = by * TY + ls % TY; ls /= TY;
         x[2] = bz * TZ + ls % TZ; ls /= TZ;
@@ -43,6 +41,7 @@ __device__ __forceinline__ void dir_info(const Geom& g, int mu, const int x[4], 
 template <typename T, int NC, class Tile>
 __global__ void __launch_bounds__(Tile::kThreads, SiteOcc<T, NC>::k5m)
 k5m_gbuild_update(Cx<T>* __restrict__ U, const Cx<T>* __restrict__ D, const DevState* st, Geom g, T half_alpha) {
+    pdl_entry();
     if (*reinterpret_cast<const volatile int*>(&st->done)) return;
     constexpr int NS = Tile::kSites;
     const int ls = threadIdx.x % NS, mu = threadIdx.x / NS;
@@ -106,18 +105,17 @@ struct SiteTileS {
 template <typename T, int NC, class Tile, int MINB>
 __global__ void __launch_bounds__(Tile::kThreads, MINB)
 k5s_gbuild_update(Cx<T>* __restrict__ U, const Cx<T>* __restrict__ D, const DevState* st, Geom g, T half_alpha) {
+    pdl_entry();
     if (*reinterpret_cast<const volatile int*>(&st->done)) return;
     constexpr int TX = Tile::tx, TY = Tile::ty, TZ = Tile::tz, TT = Tile::tt, NS = Tile::kSites, NG = Tile::NG, NR = NC / 3;
     __shared__ Cx<T> G[9 * NG];
-    int b = blockIdx.x;
-    const int x0 = (b % g.nb[0]) * TX; b /= g.nb[0];
-    const int y0 = (b % g.nb[1]) * TY; b /= g.nb[1];
-    const int z0 = (b % g.nb[2]) * TZ; b /= g.nb[2];
-    const int t0 = b * TT;
-    const long long s1 = g.L[0], s2 = s1 * g.L[1], s3 = s2 * g.L[2];
+    unsigned bz, bt;
+    split_zt(g, blockIdx.z, bz, bt);
+    const int x0 = blockIdx.x * TX, y0 = blockIdx.y * TY, z0 = bz * TZ, t0 = bt * TT;
+    const int s1 = g.L[0], s2 = s1 * g.L[1], s3 = s2 * g.L[2];      // 32-bit site arithmetic (V < 2^31)
     const int tid = threadIdx.x, ls = tid % NS, mu = tid / NS;
     const int lx = ls % TX, ly = (ls / TX) % TY, lz = (ls / (TX * TY)) % TZ, lt = ls / (TX * TY * TZ);
-    const long long s = (x0 + lx) + s1 * (y0 + ly) + s2 * (z0 + lz) + s3 * (t0 + lt);
+    const int s = (x0 + lx) + s1 * (y0 + ly) + s2 * (z0 + lz) + s3 * (t0 + lt);
     // ---- this thread's link: loads in flight during the whole g phase ----
     Su3<T> u;
     Cx<T>* p = U + (size_t)mu * NC * g.V + s;
