@@ -370,6 +370,12 @@ int upload_tables(lgf_ctx* c) {
             const long double s = sinl(3.141592653589793238462643383279502884L * (long double)j / (long double)n);
             psq[j] = (T)(4.0L * s * s);
         }
+        for (int j = n / 2 + 1; j < n; ++j) psq[j] = psq[n - j];     // exactly even in k (K3 relies on it)
+        if (mu == 3 && n <= 64)
+            for (int j = 0; j <= n / 2; ++j) {
+                if (sizeof(T) == 8) c->zt_args.psq_t_half_d[j] = (double)psq[j];
+                else c->zt_args.psq_t_half_f[j] = (float)psq[j];
+            }
         CU(cudaMemcpyAsync(c->ws + c->lo.tw[mu], tw.data(), n * sizeof(Cx<T>), cudaMemcpyHostToDevice, c->stream));
         CU(cudaMemcpyAsync(c->ws + c->lo.twi[mu], twi.data(), n * sizeof(Cx<T>), cudaMemcpyHostToDevice, c->stream));
         CU(cudaMemcpyAsync(c->ws + c->lo.psq[mu], psq.data(), n * sizeof(T), cudaMemcpyHostToDevice, c->stream));

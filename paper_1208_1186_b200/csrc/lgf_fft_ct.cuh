@@ -199,7 +199,13 @@ struct ZtArgs {
     int tiles_per_comp;               // LxLy / CX
     double scale_num;                 // p2max / V
     int x_n1, x_n2, y_n1, y_n2;       // how K2 split the x and y lines (digit-swapped spectrum order)
+    // psq_t[k] for k = 0..Lt/2, by value (read as constant-bank operands by the whole-line t pass of the pipelined K3;
+    // the table is symmetric, psq_t[Lt - k] = psq_t[k], so one quotient serves both modes); Lt <= 64
+    double psq_t_half_d[33];
+    float psq_t_half_f[33];
 };
+__device__ __forceinline__ double psq_t_half(const ZtArgs& A, int k, double) { return A.psq_t_half_d[k]; }
+__device__ __forceinline__ float psq_t_half(const ZtArgs& A, int k, float) { return A.psq_t_half_f[k]; }
 
 // K3: forward z, forward t, scale, inverse t, inverse z on CX contiguous (x,y)-plane sites.
 template <typename T, class SZ, class ST_, int CX, int NTHREADS, int MINB>

@@ -328,10 +328,13 @@ fft_zt_pipe(const Cx<T>* inB, Cx<T>* out, const ZtArgs A, const int* done) {
                     Cx<T> v[NT];
                     static_for<0, NT>([&](auto m) { v[m.value] = s[m.value * PT]; });
                     RegFft<NT, -1, T>::run(v);
-                    static_for<0, NT>([&](auto kt) {
-                        const T den = pxyz + __ldg(pt + kt.value);
-                        const T sc = (zero_xyz && kt.value == 0) ? T(0) : fast_div(num, den);
-                        v[kt.value] = sc * v[kt.value];
+                    // p^2 is even in k_t: one quotient scales modes k_t and N_t - k_t
+                    static_for<0, NT / 2 + 1>([&](auto kt) {
+                        constexpr int k = kt.value;
+                        const T den = pxyz + psq_t_half(A, k, T());
+                        const T sc = (zero_xyz && k == 0) ? T(0) : fast_div(num, den);
+                        v[k] = sc * v[k];
+                        if constexpr (k != 0 && 2 * k != NT) v[NT - k] = sc * v[NT - k];
                     });
                     RegFft<NT, +1, T>::run(v);
                     static_for<0, NT>([&](auto m) { s[m.value * PT] = v[m.value]; });
