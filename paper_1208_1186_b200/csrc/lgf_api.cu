@@ -225,7 +225,24 @@ cudaError_t launch_exc(lgf_ctx* c, const void* kernel, dim3 grid, dim3 block, vo
 
 // grid of the site kernels: (x tiles, y tiles, z tiles * t tiles); see split_zt()
 dim3 grid3(const Geom& g) { return dim3((unsigned)g.nb[0], (unsigned)g.nb[1], (unsigned)(g.nb[2] * g.nb[3])); }
-void set_magic(Geom& g) { g.nb2_magic = g.nb[2] > 1 ? (unsigned)((0x100000000ULL + (unsigned)g.nb[2] - 1) / (unsigned)g.nb[2]) : 0u; }
+unsigned magic_of(int d) { return d > 1 ? (unsigned)((0x100000000ULL + (unsigned)d - 1) / (unsigned)d) : 0u; }
+// walk order of the site kernels' (z, t) tiles (Geom::zb): z-blocks of about 16 MB of link traffic per t step once
+// a whole t-slice of links no longer fits the L2 comfortably (LGF_ZBLOCK overrides: z-tiles per block, 0 = plain order)
+void set_walk(Geom& g, int tz, size_t link_bytes_per_site) {
+    const size_t per_ztile = (size_t)g.L[0] * g.L[1] * tz * link_bytes_per_site;
+    int zb = g.nb[2];
+    if (per_ztile * (size_t)g.nb[2] > (size_t)48 << 20) {
+        zb = (int)(((size_t)16 << 20) / per_ztile);
+        if (zb < 1) zb = 1;
+    }
+    const char* e = getenv("LGF_ZBLOCK");
+    if (e) zb = atoi(e) > 0 ? atoi(e) : g.nb[2];
+    if (zb > g.nb[2]) zb = g.nb[2];
+    while (g.nb[2] % zb) --zb;
+    g.zb = zb;
+    g.zb_magic = magic_of(zb);
+    g.nb3_magic = magic_of(g.nb[3]);
+}
 
 DevState* dev_state(lgf_ctx* c) { return reinterpret_cast<DevState*>(c->ws + c->lo.state); }
 
@@ -801,7 +818,7 @@ static int create_common(const int32_t L[4], int precision, int storage, void* w
         c->lo.nblocks_site = n;
     }
     for (int i = 0; i < 4; ++i) { c->geom.L[i] = L[i]; c->geom.nb[i] = c->lo.nb[i]; }
-    set_magic(c->geom);
+    set_walk(c->geom, kSiteTileDims[c->site_tile][2], (size_t)4 * storage * c->wbytes);
     c->geom.V = c->V;
     {   // K5 flavour: 0 = thread per (site, direction), 1 = thread per site (LGF_SITE_VARIANT / LGF_SITEMU_TILE: A/B knobs)
         const char* e = getenv("LGF_SITE_VARIANT");
@@ -819,7 +836,7 @@ static int create_common(const int32_t L[4], int precision, int storage, void* w
     }
     c->geom_mu = c->geom;
     for (int i = 0; i < 4; ++i) c->geom_mu.nb[i] = c->lo.nbm[i];
-    set_magic(c->geom_mu);
+    set_walk(c->geom_mu, kMuTileDims[c->mu_tile][2], (size_t)8 * storage * c->wbytes);
     const int mu_default_fallback = ((precision == LGF_F64 && storage == LGF_REAL18) || (precision == LGF_F32 && storage == LGF_REAL12)) ? 0 : 1;
     {   // shared-g K5 (LGF_SITE_VARIANT=2, LGF_SITES_TILE): needs every extent to be a multiple of the tile's
         const char* e = getenv("LGF_SITES_TILE");
@@ -836,7 +853,7 @@ static int create_common(const int32_t L[4], int precision, int storage, void* w
             n *= c->geom_s.nb[i] > 0 ? c->geom_s.nb[i] : 1;
         }
         c->nblocks_s = n;
-        set_magic(c->geom_s);
+        set_walk(c->geom_s, kSTileDims[t][2], (size_t)8 * storage * c->wbytes);
         if (c->site_variant == 2 && !ok) c->site_variant = mu_default_fallback;
 
     }

@@ -15,15 +15,23 @@ struct Geom {
     int L[4];    // Lx, Ly, Lz, Lt
     int nb[4];   // tiles per axis for the per-site kernels; launched as a (nb0, nb1, nb2 * nb3) grid
     long long V;
-    unsigned int nb2_magic;   // ceil(2^32 / nb2): blockIdx.z / nb2 by one multiply (see split_zt)
+    // walk order of the (z, t) tiles: blockIdx.z = (zblk * nb3 + bt) * zb + zi, bz = zblk * zb + zi.  zb = nb2 is the
+    // plain order (t slowest).  On lattices whose t-slice of links outgrows the L2 (64^4: 100 MB) a z-block of
+    // zb tiles is walked through all t before the next z-block starts, so that the t-neighbour data (backward
+    // links in K1, forward Delta~ in K5) is re-read from L2 one z-block later, not from DRAM one t-slice later.
+    int zb;
+    unsigned int zb_magic, nb3_magic;     // ceil(2^32 / zb), ceil(2^32 / nb3)  (0 when the divisor is 1)
 };
 
 // The site kernels are launched on a 3-D grid (x tiles, y tiles, z tiles * t tiles): same CTA order as a linear
 // grid, but no runtime integer divisions in the prologue (they were ~100 of k5s's ~600 instructions per thread
-// and sat in front of the first load).  bzt < 2^16 and nb2 < 2^16, so the multiply-high quotient is exact.
+// and sat in front of the first load).  All operands are < 2^16, so the multiply-high quotients are exact.
+__device__ __forceinline__ unsigned div_magic(unsigned n, unsigned magic) { return magic ? __umulhi(n, magic) : n; }
 __device__ __forceinline__ void split_zt(const Geom& g, unsigned bzt, unsigned& bz, unsigned& bt) {
-    bt = g.nb[2] == 1 ? bzt : __umulhi(bzt, g.nb2_magic);
-    bz = bzt - bt * (unsigned)g.nb[2];
+    const unsigned q = div_magic(bzt, g.zb_magic), zi = bzt - q * (unsigned)g.zb;
+    const unsigned zblk = div_magic(q, g.nb3_magic);
+    bt = q - zblk * (unsigned)g.nb[3];
+    bz = zblk * (unsigned)g.zb + zi;
 }
 __device__ __forceinline__ unsigned linear_block() { return blockIdx.x + gridDim.x * (blockIdx.y + gridDim.y * blockIdx.z); }
 
@@ -84,11 +92,12 @@ __device__ __forceinline__ long long axis_stride(const Geom& g, int mu) {
 }
 
 // Load one link into registers; in 12-real mode rebuild row 2.
-// STREAM: this is the last use of the link in the kernel (L2 evict-first); otherwise a plain load.
-template <typename T, int NC, bool STREAM = false>
-__device__ __forceinline__ void load_link(Su3<T>& u, const Cx<T>* __restrict__ U, long long V, int mu, long long s) {
+// stream: this is the last use of the link in the kernel (L2 evict-first); otherwise a plain load
+// (stream is a compile-time constant at every call site once the direction loops are unrolled)
+template <typename T, int NC>
+__device__ __forceinline__ void load_link(Su3<T>& u, const Cx<T>* __restrict__ U, long long V, int mu, long long s, int stream = 0) {
     const Cx<T>* p = U + (size_t)mu * NC * V + s;
-    if (STREAM) {
+    if (stream) {
         const uint64_t pol = l2_evict_first_policy();
 #pragma unroll
         for (int c = 0; c < NC; ++c) u.m[c] = ld_cx_stream(p + (size_t)c * V, pol);
@@ -156,7 +165,7 @@ k1_delta_theta_F(const Cx<T>* __restrict__ U, Cx<T>* __restrict__ D, double2* __
             // L2 for K2) and hurt in fp64 (122 -> 134 us, 18-real: the backward re-reads start missing L2)
             {
                 Su3<T> a;
-                load_link<T, NC, sizeof(T) == 4>(a, U, g.V, mu, s);
+                load_link<T, NC>(a, U, g.V, mu, s, sizeof(T) == 4);
                 c0 = c0 - (a.m[1] - conj(a.m[3]));
                 c1 = c1 - (a.m[2] - conj(a.m[6]));
                 c2 = c2 - (a.m[5] - conj(a.m[7]));
@@ -165,7 +174,7 @@ k1_delta_theta_F(const Cx<T>* __restrict__ U, Cx<T>* __restrict__ D, double2* __
             }
             {
                 Su3<T> b;
-                load_link<T, NC, sizeof(T) == 4>(b, U, g.V, mu, sb);
+                load_link<T, NC>(b, U, g.V, mu, sb, sizeof(T) == 4);
                 c0 = c0 + (b.m[1] - conj(b.m[3]));
                 c1 = c1 + (b.m[2] - conj(b.m[6]));
                 c2 = c2 + (b.m[5] - conj(b.m[7]));

@@ -266,6 +266,31 @@ def test_generic_and_compile_time_fft_paths_agree(monkeypatch):
         gf.close()
 
 
+@pytest.mark.parametrize("zb", ["1", "2"])
+@pytest.mark.parametrize("L", [(16, 16, 8, 8), (8, 8, 16, 16), (6, 4, 12, 8)])
+def test_zblock_walk_order(monkeypatch, L, zb):
+    """The site kernels' z-blocked (z-block outer, t inner) CTA order used on lattices whose t-slice outgrows
+    the L2 (LGF_ZBLOCK forces it on small ones): same links, theta and F as the oracle, in every mode."""
+    monkeypatch.setenv("LGF_ZBLOCK", zb)
+    U = gi.make_config(L, 37, 0.59)
+    ref, thh, Fh = oracle.iterate(L, U, 2, ALPHA)
+    for prec, stor in MODES:
+        gf = _fixer(L, prec, stor, U)
+        r = gf.iterate(2, ALPHA)
+        assert np.max(np.abs(_cplx(gf.store()) - ref)) <= 1e-12
+        assert abs(r.theta - thh[2]) <= 1e-10 * thh[2] and abs(r.F - Fh[2]) <= 1e-12
+        gf.close()
+    U32 = gi.as_real(U, torch.float32)
+    ref32, _, Fh32 = oracle.iterate(L, gi.from_real(U32), 2, ALPHA)
+    for stor in (lgf.LGF_REAL12, lgf.LGF_REAL18):
+        gf = lgf.GaugeFixer(L, lgf.LGF_F32, stor)
+        gf.load(U32)
+        r = gf.iterate(2, ALPHA)
+        assert np.max(np.abs(_cplx(gf.store()) - ref32)) <= 2e-5
+        assert abs(r.F - Fh32[2]) <= 1e-5 * abs(Fh32[2])
+        gf.close()
+
+
 @pytest.mark.parametrize("L", [(8, 8, 8, 8), (16, 16, 8, 8), (32, 8, 4, 8)])
 @pytest.mark.parametrize("prec,stor", MODES)
 def test_fused_update_kernel(monkeypatch, L, prec, stor):
