@@ -54,7 +54,7 @@ template <typename T, int NC> struct SiteOcc {
 #ifdef LGF_K1_OCC
     static constexpr int k1 = LGF_K1_OCC;
 #else
-    static constexpr int k1 = sizeof(T) == 8 ? 2 : 3;
+    static constexpr int k1 = sizeof(T) == 8 ? 2 : 4;     // fp32 at 4 (64 registers): K1 65.7 -> 61.6 us 18-real, 52.6 -> 49.2 us 12-real at 32^4
 #endif
     static constexpr int k5 = sizeof(T) == 8 ? 2 : (NC == 6 ? 4 : 2);
     static constexpr int k5m = sizeof(T) == 8 ? 2 : 3;
