@@ -27,6 +27,16 @@ def _cplx(t):
     return torch.view_as_complex(t.to(torch.float64).contiguous()).numpy()
 
 
+def _max_abs_diff(a, b, chunk=1 << 20):
+    """max |a - b| over two equally shaped complex arrays, in chunks (64^4: no 10 GB temporaries)."""
+    a = a.reshape(-1)
+    b = b.reshape(-1)
+    m = 0.0
+    for i in range(0, a.size, chunk * 36):
+        m = max(m, float(np.max(np.abs(a[i:i + chunk * 36] - b[i:i + chunk * 36]))))
+    return m
+
+
 def _fixer(L, prec, stor, U):
     dt = torch.float64 if prec == lgf.LGF_F64 else torch.float32
     gf = lgf.GaugeFixer(L, prec, stor)
@@ -337,4 +347,38 @@ def test_large_extent_fft_kernels(L):
     r = gf.iterate(2, ALPHA)
     assert np.max(np.abs(_cplx(gf.store()) - ref32)) <= 2e-5
     assert abs(r.F - Fh32[2]) <= 1e-5 * abs(Fh32[2])
+    gf.close()
+
+
+def test_full_size_64x4_one_iteration():
+    """configs[4] at its full size, 64^4 (16.8 M sites, 9.7 GB of fp64 links), in the launch configuration bench.py
+    times there and nowhere smaller: K3 on the half-tile ring, K2/K4 on 64x64 two-stage planes, the site kernels in
+    the z-blocked walk order.  Every link after one iteration against the oracle, element by element (fp64, both
+    storage modes), the initial theta and F, and the fp32 12-real path against the oracle fed the rounded field.
+    About a minute of host time: the oracle transforms 9 x 16.8 M complex numbers."""
+    L = (64, 64, 64, 64)
+    U = gi.make_config(L, gi.CONFIG_SEED + 4, 0.59, device="cuda")
+    Ur = gi.as_real(U).cpu()
+    ref, thh, Fh = oracle.iterate(L, Ur, 1, ALPHA)
+    for stor in (lgf.LGF_REAL12, lgf.LGF_REAL18):
+        gf = lgf.GaugeFixer(L, lgf.LGF_F64, stor)
+        gf.load(Ur)
+        r0 = gf.measure()
+        assert abs(r0.theta - thh[0]) <= 1e-12 * thh[0] and abs(r0.F - Fh[0]) <= 1e-12
+        r = gf.iterate(1, ALPHA)
+        got = _cplx(gf.store())
+        assert _max_abs_diff(got, ref) <= 1e-12
+        assert abs(r.theta - thh[1]) <= 1e-11 * thh[1] and abs(r.F - Fh[1]) <= 1e-12
+        gf.close()
+        del got
+    del ref
+    U32 = Ur.to(torch.float32)
+    del Ur, U
+    torch.cuda.empty_cache()
+    ref32, _, Fh32 = oracle.iterate(L, U32.to(torch.float64), 1, ALPHA)
+    gf = lgf.GaugeFixer(L, lgf.LGF_F32, lgf.LGF_REAL12)
+    gf.load(U32)
+    r = gf.iterate(1, ALPHA)
+    assert _max_abs_diff(_cplx(gf.store()), ref32) <= 2e-5
+    assert abs(r.F - Fh32[1]) <= 1e-5 * abs(Fh32[1])
     gf.close()
