@@ -413,20 +413,16 @@ struct Impl {
 
     static int k1(lgf_ctx* c, int mode) {
         double2* partials = reinterpret_cast<double2*>(c->ws + c->lo.partials);
-        int nblocks;
-        {
-            nblocks = c->lo.nblocks_site;
-#define LGF_K1_CASE(ID, TILE) case ID: launch_ex(c, k1_delta_theta_F<T, NC, TILE>, grid3(c->geom), dim3(TILE::kThreads), 0,  \
-                links(c), delta_src(c), partials, dev_state(c), c->geom, mode); break;
-            switch (c->site_tile) {
-                LGF_K1_CASE(1, Tile1) LGF_K1_CASE(2, Tile2) LGF_K1_CASE(3, Tile3) LGF_K1_CASE(4, Tile4) LGF_K1_CASE(5, Tile5)
-                default: launch_ex(c, k1_delta_theta_F<T, NC, Tile0>, grid3(c->geom), dim3(Tile0::kThreads), 0, 
-                    links(c), delta_src(c), partials, dev_state(c), c->geom, mode);
-            }
-#undef LGF_K1_CASE
+#define LGF_K1_CASE(ID, TILE) case ID: launch_ex(c, k1_delta_theta_F<T, NC, TILE>, grid3(c->geom), dim3(TILE::kThreads), 0, \
+            links(c), delta_src(c), partials, dev_state(c), c->geom, mode); break;
+        switch (c->site_tile) {
+            LGF_K1_CASE(1, Tile1) LGF_K1_CASE(2, Tile2) LGF_K1_CASE(3, Tile3) LGF_K1_CASE(4, Tile4) LGF_K1_CASE(5, Tile5)
+            default: launch_ex(c, k1_delta_theta_F<T, NC, Tile0>, grid3(c->geom), dim3(Tile0::kThreads), 0,
+                links(c), delta_src(c), partials, dev_state(c), c->geom, mode);
         }
+#undef LGF_K1_CASE
         CU(cudaGetLastError());
-        launch_ex(c, k1_finish, dim3(1), dim3(kFinishThreads), 0, partials, nblocks, dev_state(c), (double)c->V, mode);
+        launch_ex(c, k1_finish, dim3(1), dim3(kFinishThreads), 0, partials, c->lo.nblocks_site, dev_state(c), (double)c->V, mode);
         c->launches += 2;
         CU(cudaGetLastError());
         return LGF_OK;
