@@ -256,6 +256,7 @@ def main():
             "site_updates_per_s": world * K * V / (ms * 1e-3),
             "algorithmic_GBps": b_iter * V * K / (ms * 1e-3) / 1e9,
             "frac_of_hbm_peak": b_iter * V * K / (ms * 1e-3) / 1e9 / peak,
+            "frac_of_nominal_8TBps": b_iter * V * K / (ms * 1e-3) / 1e9 / 8000.0,   # north_star's nominal figure
             "bytes_per_site_iteration": b_iter, "theta": res.theta, "F": res.F,
             "launches": launches, "kernels": kernels,
         }
@@ -322,6 +323,7 @@ def main():
             "site_updates_per_s": pr["site_updates_per_s"],
             "achieved_HBM_GBps_algorithmic": pr["algorithmic_GBps"],
             "iteration_frac_of_hbm_roofline": pr["frac_of_hbm_peak"],
+            "iteration_frac_of_nominal_8TBps": pr["frac_of_nominal_8TBps"],
             "roofline": {"bound": "hbm", "kernel": dom[0], "achieved": dom[1]["algorithmic_GBps"], "peak": peak,
                          "unit": "GB/s", "frac": dom[1]["frac_of_peak"], "traffic": ncu_traffic(mode_key, dom[0]),
                          "algorithmic_bytes_per_launch": dom_bytes, "peak_source": peak_src},

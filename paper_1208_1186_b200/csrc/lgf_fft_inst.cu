@@ -62,10 +62,10 @@ static const XyPipeEntry* xyp_tab(int precision, int* n) { return precision ? xy
 static const ZtPipeEntry* ztp_tab(int precision, int* n) { return precision ? zt_pipe_table_f64(n) : zt_pipe_table_f32(n); }
 
 // K4 may run on a different tile shape than K2 (both read and write the natural layout on their own):
-// LGF_XYP_INV_VARIANT = v picks the v-th match; default -1 = "same entry as K2" unless a tuned default exists.
+// LGF_XYP_INV_VARIANT = v picks the v-th match; default: the same entry as K2.
 const XyPipeEntry* find_xy_pipe_inv(int precision, int nx, int ny, const XyPipeEntry* fwd) {
     const char* e = getenv("LGF_XYP_INV_VARIANT");
-    int skip = e ? atoi(e) : ((precision == 1 && nx == 32 && ny == 32 && !getenv("LGF_XYP_VARIANT")) ? 1 : -1);
+    int skip = e ? atoi(e) : -1;
     if (skip < 0) return fwd;
     int n = 0;
     const XyPipeEntry* t = xyp_tab(precision, &n);
