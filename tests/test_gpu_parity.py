@@ -382,3 +382,65 @@ def test_full_size_64x4_one_iteration():
     assert _max_abs_diff(_cplx(gf.store()), ref32) <= 2e-5
     assert abs(r.F - Fh32[1]) <= 1e-5 * abs(Fh32[1])
     gf.close()
+
+
+def _fix_vs_oracle(L, seed, prec, stor, plaq):
+    """lgf_fix to theta < 1e-15 at a full-size config against oracle.fix on the same field: identical iteration
+    count, theta within relative 1e-10 plus the derived rounding floor, F relative 1e-10, links."""
+    U = gi.make_config(L, seed, plaq, device="cuda").cpu()
+    ref, n, theta, F, thh, Fh = oracle.fix(L, U, ALPHA, 1e-15, 5000)
+    gf = _fixer(L, prec, stor, U)
+    r = gf.fix(ALPHA, 1e-15, 5000)
+    assert r.iterations == n and r.converged, (r.iterations, n)
+    got = _cplx(gf.store())
+    d_rms = float(np.sqrt(np.mean(np.abs(got - ref) ** 2)))
+    sigma = 2.0 * np.sqrt(8.0 * theta / (3.0 * gi.volume(L))) * d_rms
+    assert d_rms < 1e-14
+    assert abs(r.theta - theta) <= 1e-10 * theta + 6.0 * sigma, (r.theta, theta, d_rms, sigma)
+    assert abs(r.F - F) <= 1e-10 * F
+    assert _max_abs_diff(got, ref) <= 1e-11
+    # F never decreases along the way (pin P6 on the GPU trajectory), theta well above the floor tracks the oracle
+    gf.load(gi.as_real(U))
+    k = min(20, n - 1)
+    rk = gf.fix(ALPHA, 1e-30, k)
+    assert rk.iterations == k and abs(rk.theta - thh[k]) <= 1e-10 * thh[k] and abs(rk.F - Fh[k]) <= 1e-12
+    gf.close()
+
+
+def test_config2_fix_32x4_fp64_12():
+    """configs[2]: the 32^4 fp64 run to theta < 1e-15 (12-real, the headline mode), full size, vs the oracle."""
+    _fix_vs_oracle((32, 32, 32, 32), gi.CONFIG_SEED + 2, lgf.LGF_F64, lgf.LGF_REAL12, 0.59)
+
+
+def test_config3_fix_48x3x8_fp64_12():
+    """configs[3]: 48^3 x 8 (radix-3 lines along x, y, z), fp64 12-real, plaquette 0.58, to theta < 1e-15, full size."""
+    _fix_vs_oracle((48, 48, 48, 8), gi.CONFIG_SEED + 3, lgf.LGF_F64, lgf.LGF_REAL12, 0.58)
+
+
+def test_config2_fp32_1000_iterations_properties():
+    """configs[2]'s fixed 1000-iteration fp32 run at 32^4 in both storage modes: what must hold at any size without
+    an oracle run of that length -- every link still unitary with det 1 to the fp32 bar (2e-5, no re-projection:
+    reading #14), the mean plaquette of the result equal to the input's (gauge invariance, pin P5), F not below
+    the fp64 value reached by the converged fp64 run minus the fp32 bar, theta at the fp32 floor."""
+    L = (32, 32, 32, 32)
+    U = gi.make_config(L, gi.CONFIG_SEED + 2, 0.59, device="cuda")
+    plaq0 = gi.mean_plaquette(U, L)
+    U32 = gi.as_real(U, torch.float32)
+    gf64 = lgf.GaugeFixer(L, lgf.LGF_F64, lgf.LGF_REAL12)
+    gf64.load(gi.as_real(U))
+    r64 = gf64.fix(ALPHA, 1e-15, 5000)
+    gf64.close()
+    for stor in (lgf.LGF_REAL12, lgf.LGF_REAL18):
+        gf = lgf.GaugeFixer(L, lgf.LGF_F32, stor)
+        gf.load(U32)
+        r = gf.iterate(1000, ALPHA)
+        out = gi.from_real(gf.store(device="cuda").to(torch.float64))
+        gf.close()
+        eye = torch.eye(3, dtype=out.dtype, device=out.device)
+        uni = (out @ out.conj().transpose(-1, -2) - eye).abs().max().item()
+        det = (torch.linalg.det(out) - 1).abs().max().item()
+        assert uni <= 2e-5 and det <= 2e-5, (uni, det)
+        assert abs(gi.mean_plaquette(out, L) - plaq0) <= 2e-5
+        assert abs(r.F - r64.F) <= 1e-5 * r64.F
+        assert r.theta < 1e-12
+        del out
