@@ -191,6 +191,12 @@ struct lgf_ctx {
     // programmatic dependent launch: set while the iteration body is captured, so that every kernel after the
     // first becomes a programmatic edge of the graph (its CTAs are scheduled while the previous kernel drains
     // and block in griddepcontrol.wait, see pdl_entry()); LGF_PDL=0 turns it off
+    // deferred k1_finish: the end-of-iteration reduction runs on a second graph branch beside the next iteration's
+    // K2 (which is then not gated by `done`: it only writes the spectrum buffer) and once after the last iteration
+    // of a batch; LGF_DEFER_FINISH=0 puts it back behind K1
+    bool defer_finish;
+    cudaStream_t fin_stream;
+    cudaEvent_t ev_fork, ev_join;
     bool pdl_enabled, pdl;
     int pdl_mask, pdl_idx;       // which launches of the body (bit i: i-th launch) carry the attribute
 };
@@ -251,6 +257,7 @@ __global__ void init_state_kernel(DevState* st, double tol, long long max_iter) 
     st->iter = 0;
     st->done = 0;
     st->ticket = 0;
+    st->pending = 0;
     st->tol = tol;
     st->max_iter = max_iter;
 }
@@ -411,7 +418,7 @@ struct Impl {
     static Cx<T>* delta_src(lgf_ctx* c) { return reinterpret_cast<Cx<T>*>(c->ws + (c->fused_tile >= 0 ? c->lo.delta3 : c->lo.delta)); }
     static Cx<T>* staging(lgf_ctx* c) { return reinterpret_cast<Cx<T>*>(c->ws + c->lo.staging); }
 
-    static int k1(lgf_ctx* c, int mode) {
+    static int k1(lgf_ctx* c, int mode, bool with_finish = true) {
         double2* partials = reinterpret_cast<double2*>(c->ws + c->lo.partials);
 #define LGF_K1_CASE(ID, TILE) case ID: launch_ex(c, k1_delta_theta_F<T, NC, TILE>, grid3(c->geom), dim3(TILE::kThreads), 0, \
             links(c), delta_src(c), partials, dev_state(c), c->geom, mode); break;
@@ -422,8 +429,14 @@ struct Impl {
         }
 #undef LGF_K1_CASE
         CU(cudaGetLastError());
+        c->launches++;
+        return with_finish ? k1_reduce(c, mode) : LGF_OK;
+    }
+    // k1_finish on the context's stream (mode 3: deferred, see lgf_ctx::defer_finish)
+    static int k1_reduce(lgf_ctx* c, int mode) {
+        double2* partials = reinterpret_cast<double2*>(c->ws + c->lo.partials);
         launch_ex(c, k1_finish, dim3(1), dim3(kFinishThreads), 0, partials, c->lo.nblocks_site, dev_state(c), (double)c->V, mode);
-        c->launches += 2;
+        c->launches++;
         CU(cudaGetLastError());
         return LGF_OK;
     }
@@ -699,14 +712,28 @@ int enqueue_iteration_body(lgf_ctx* c, double alpha) {
     int rc;
     c->pdl = false;                 // the first kernel of the graph has no predecessor to overlap with
     c->pdl_idx = 0;
-    if ((rc = DISPATCH(c, fft(c, 0, true)))) return rc;
+    const bool defer = c->defer_finish && c->fused_tile < 0;
+    if (defer) {
+        // second branch: fold the previous iteration's partials into theta / F / iter / done while K2 runs
+        cudaStream_t main_stream = c->stream;
+        CU(cudaEventRecord(c->ev_fork, main_stream));
+        CU(cudaStreamWaitEvent(c->fin_stream, c->ev_fork, 0));
+        c->stream = c->fin_stream;
+        rc = DISPATCH(c, k1_reduce(c, 3));
+        c->stream = main_stream;
+        if (rc) return rc;
+        CU(cudaEventRecord(c->ev_join, c->fin_stream));
+        c->pdl_idx = 0;
+    }
+    if ((rc = DISPATCH(c, fft(c, 0, !defer)))) return rc;
+    if (defer) CU(cudaStreamWaitEvent(c->stream, c->ev_join, 0));
     cudaStreamCaptureStatus cs = cudaStreamCaptureStatusNone;
     if (cudaStreamIsCapturing(c->stream, &cs) == cudaSuccess && cs == cudaStreamCaptureStatusActive) c->pdl = c->pdl_enabled;
     if ((rc = DISPATCH(c, fft(c, 1, true)))) return rc;
     if ((rc = DISPATCH(c, fft(c, 2, true)))) return rc;
     if (c->fused_tile >= 0) return DISPATCH(c, k51(c, alpha));
     if ((rc = DISPATCH(c, k5(c, alpha)))) return rc;
-    if ((rc = DISPATCH(c, k1(c, 1)))) return rc;
+    if ((rc = DISPATCH(c, k1(c, 1, !defer)))) return rc;
     return LGF_OK;
 }
 
@@ -739,6 +766,7 @@ int enqueue_iterations(lgf_ctx* c, int64_t n) {
         CU(cudaGraphLaunch(c->graph, c->stream));
         c->launches += c->launches_per_iter;
     }
+    if (n > 0 && c->defer_finish && c->fused_tile < 0) return DISPATCH(c, k1_reduce(c, 3));   // the last iteration's
     return LGF_OK;
 }
 
@@ -864,6 +892,14 @@ static int create_common(const int32_t L[4], int precision, int storage, void* w
         cudaError_t e = cudaStreamCreateWithFlags(&c->cap_stream, cudaStreamNonBlocking);
         if (e != cudaSuccess) rc = cuda_fail(e, "cudaStreamCreateWithFlags");
     }
+    if (!rc) {
+        const char* e = getenv("LGF_DEFER_FINISH");
+        c->defer_finish = !(e && atoi(e) == 0);
+        cudaError_t ce = cudaStreamCreateWithFlags(&c->fin_stream, cudaStreamNonBlocking);
+        if (ce == cudaSuccess) ce = cudaEventCreateWithFlags(&c->ev_fork, cudaEventDisableTiming);
+        if (ce == cudaSuccess) ce = cudaEventCreateWithFlags(&c->ev_join, cudaEventDisableTiming);
+        if (ce != cudaSuccess) rc = cuda_fail(ce, "deferred-finish stream/events");
+    }
     for (int i = 0; i < 2 && !rc; ++i) {
         cudaError_t e = cudaEventCreateWithFlags(&c->ev[i], cudaEventDisableTiming);
         if (e != cudaSuccess) rc = cuda_fail(e, "cudaEventCreate");
@@ -906,6 +942,9 @@ int lgf_destroy(lgf_ctx* c) {
     if (c->stream || c->ws) cudaStreamSynchronize(c->stream);
     if (c->graph) cudaGraphExecDestroy(c->graph);
     if (c->cap_stream) cudaStreamDestroy(c->cap_stream);
+    if (c->fin_stream) cudaStreamDestroy(c->fin_stream);
+    if (c->ev_fork) cudaEventDestroy(c->ev_fork);
+    if (c->ev_join) cudaEventDestroy(c->ev_join);
     for (int i = 0; i < 2; ++i)
         if (c->ev[i]) cudaEventDestroy(c->ev[i]);
     if (c->host_state) cudaFreeHost(c->host_state);

@@ -45,7 +45,7 @@ struct DevState {
     double tol;
     long long max_iter;
     int cur;                 // which of the two link buffers holds the current field (fused path swaps them)
-    int pad_;
+    int pending;             // K1 has written the partials of an applied update that k1_finish has not folded in yet
 };
 
 // Resident CTAs per SM each site kernel is compiled for (= register cap 65536 / (256 * n)); measured
@@ -141,9 +141,10 @@ __device__ __forceinline__ void block_sum2(double& a, double& b) {
 template <typename T, int NC, class Tile>
 __global__ void __launch_bounds__(Tile::kThreads, SiteOcc<T, NC>::k1)
 k1_delta_theta_F(const Cx<T>* __restrict__ U, Cx<T>* __restrict__ D, double2* __restrict__ partials,
-                 const DevState* st, Geom g, int mode) {
+                 DevState* st, Geom g, int mode) {
     pdl_entry();
     if (mode == 1 && *reinterpret_cast<const volatile int*>(&st->done)) return;
+    if (mode == 1 && threadIdx.x == 0 && linear_block() == 0) st->pending = 1;    // folded in by the next k1_finish
     int x[4];
 #ifndef LGF_K1_FORWARD
     const bool valid = Tile::template coords<true>(g, x);
@@ -209,6 +210,9 @@ __global__ void __launch_bounds__(kFinishThreads)
 k1_finish(const double2* __restrict__ partials, int n, DevState* st, double V, int mode) {
     pdl_entry();
     if (mode >= 1 && *reinterpret_cast<volatile int*>(&st->done)) return;
+    // mode 3: deferred end of an iteration -- launched beside the NEXT iteration's K2 (and once after the last
+    // iteration of a batch); a no-op when the previous K1 has been folded in already
+    if (mode == 3 && !*reinterpret_cast<volatile int*>(&st->pending)) return;
     double a = 0.0, b = 0.0;
     for (int i = threadIdx.x; i < n; i += kFinishThreads) {
         const double2 p = partials[i];
@@ -221,6 +225,7 @@ k1_finish(const double2* __restrict__ partials, int n, DevState* st, double V, i
         st->theta = theta;
         st->F = b / (12.0 * V);
         if (mode >= 1) {
+            st->pending = 0;
             const long long it = st->iter + 1;
             st->iter = it;
             if (mode == 2) st->cur ^= 1;     // fused update: the new links were written to the other buffer
