@@ -712,7 +712,9 @@ int enqueue_iteration_body(lgf_ctx* c, double alpha) {
     int rc;
     c->pdl = false;                 // the first kernel of the graph has no predecessor to overlap with
     c->pdl_idx = 0;
-    const bool defer = c->defer_finish && c->fused_tile < 0;
+    // only with the pipelined FFT path, whose K2 is out of place: an ungated in-place K2 (generic / one-tile-per-CTA
+    // kernels) would overwrite Delta in the no-op iterations that follow the crossing inside a batch
+    const bool defer = c->defer_finish && c->fused_tile < 0 && c->xy_pipe != nullptr;
     if (defer) {
         // second branch: fold the previous iteration's partials into theta / F / iter / done while K2 runs
         cudaStream_t main_stream = c->stream;
@@ -766,7 +768,7 @@ int enqueue_iterations(lgf_ctx* c, int64_t n) {
         CU(cudaGraphLaunch(c->graph, c->stream));
         c->launches += c->launches_per_iter;
     }
-    if (n > 0 && c->defer_finish && c->fused_tile < 0) return DISPATCH(c, k1_reduce(c, 3));   // the last iteration's
+    if (n > 0 && c->defer_finish && c->fused_tile < 0 && c->xy_pipe != nullptr) return DISPATCH(c, k1_reduce(c, 3));   // the last iteration's
     return LGF_OK;
 }
 

@@ -444,3 +444,27 @@ def test_config2_fp32_1000_iterations_properties():
         assert abs(r.F - r64.F) <= 1e-5 * r64.F
         assert r.theta < 1e-12
         del out
+
+
+@pytest.mark.parametrize("L", [(8, 8, 8, 8), (6, 4, 12, 8), (16, 8, 4, 12), (16, 16, 8, 8)])
+def test_iterate_after_fix_without_reload(L):
+    """lgf_fix converges in the middle of a batch of enqueued iterations; the no-op iterations behind the crossing
+    must leave Delta of the final links intact, because a following lgf_iterate reuses it (pipelined, one-tile-per-CTA
+    and generic FFT paths).  Reference: a fresh context loaded with the stored links."""
+    U = gi.make_config(L, 43, 0.59)
+    gf = _fixer(L, lgf.LGF_F64, lgf.LGF_REAL12, U)
+    for tol in (1e-6, 3e-7, 1e-7):                        # a tolerance whose crossing falls inside a batch of 8
+        gf.load(gi.as_real(U))
+        r = gf.fix(ALPHA, tol, 5000)
+        if r.iterations % 8 != 0:
+            break
+    assert r.converged and r.iterations % 8 != 0
+    mid = gf.store()
+    ra = gf.iterate(3, ALPHA)
+    after = gf.store()
+    gf.close()
+    gf2 = lgf.GaugeFixer(L, lgf.LGF_F64, lgf.LGF_REAL12)
+    gf2.load(mid)
+    rb = gf2.iterate(3, ALPHA)
+    assert ra.theta == rb.theta and ra.F == rb.F and torch.equal(after, gf2.store())
+    gf2.close()
