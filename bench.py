@@ -10,6 +10,11 @@ PAPER.md:72-74), the other three precision x storage modes are reported in "mode
   python bench.py --gpus N --steps K --warmup W                 # this repo's CUDA path
   python bench.py --impl reference --gpus N --steps K --warmup W  # the oracle on the host cores
 
+The same line carries, under "lattices", the other headline shapes north_star names -- 48^3 x 8
+(configs[3]) and 64^4 (configs[4]) -- in all four precision x storage modes (whole-iteration time
+from CUDA events around K graph-replayed iterations, per-kernel times from lgf_profile_iterate,
+each as a fraction of the measured and of the nominal 8 TB/s HBM roofline); `--lattices none` skips them.
+
 N > 1 (torchrun): "replicas only" -- every rank fixes its own lattice, no data-path collective
 (SURVEY.md §8(e)); value = N*K iterations / max-over-ranks device time.
 """
@@ -42,6 +47,9 @@ def parse_args():
     ap.add_argument("--storage", type=int, default=12, choices=[12, 18])
     ap.add_argument("--modes", default="all", choices=["all", "primary"],
                     help="all: also time the other three precision/storage modes")
+    ap.add_argument("--lattices", default="48,48,48,8;64,64,64,64",
+                    help="';'-separated extra lattices timed in all four modes under the 'lattices' key ('none' = skip)")
+    ap.add_argument("--lattice-steps", type=int, default=20, help="timed iterations per mode on the extra lattices")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--plaquette", type=float, default=0.59)
@@ -67,26 +75,36 @@ def measured_peak():
         return FALLBACK_HBM_GBS, "fallback (B200_PROFILING.md 6.65 TB/s)"
 
 
-def ncu_traffic(mode_key: str, kernel: str):
-    """dram bytes per launch from the committed ncu --set full capture, or None."""
+def ncu_traffic(lattice_key: str, mode_key: str, kernel: str):
+    """(dram bytes per launch, provenance) of one kernel from the committed `ncu --set full` captures
+    (profiles/ncu_traffic.json: dram__bytes_read.sum + dram__bytes_write.sum per launch, with the capture file and the
+    commit each figure was taken at), or (None, None) if that kernel / mode / lattice has no capture."""
     try:
         t = json.load(open(os.path.join(ROOT, "profiles", "ncu_traffic.json")))
-        return t.get(mode_key, {}).get(kernel)
+        e = t.get(lattice_key, {}).get(mode_key, {})
+        v = e.get("kernels", {}).get(kernel)
+        if v is None:
+            return None, None
+        return v, {"file": e.get("file"), "commit": e.get("commit"), "metric": "dram__bytes_read.sum + dram__bytes_write.sum per launch"}
     except Exception:
-        return None
+        return None, None
 
 
 class ClockSampler:
+    """nvidia-smi clock / throttle-reason samples every 50 ms, from before the warm-up of the first mode until the last
+    timed loop has ended.  The driver's `--steps 20` timed region is only a few milliseconds long, so main() keeps the
+    primary mode's iteration loop running (untimed, same kernels) until at least kMinLoadSeconds of load have been sampled."""
     Q = ("clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.hw_slowdown,"
          "clocks_event_reasons.hw_thermal_slowdown,clocks_event_reasons.sw_thermal_slowdown,"
          "clocks_event_reasons.sw_power_cap")
+    kMinLoadSeconds = 1.5
 
     def __init__(self, index: int):
         self.f = tempfile.NamedTemporaryFile("w+", suffix=".csv", delete=False)
         self.p = None
         try:
             self.p = subprocess.Popen(["nvidia-smi", "-i", str(index), f"--query-gpu={self.Q}",
-                                       "--format=csv,noheader,nounits", "-lms", "100"],
+                                       "--format=csv,noheader,nounits", "-lms", "50"],
                                       stdout=self.f, stderr=subprocess.DEVNULL)
         except Exception:
             self.p = None
@@ -102,16 +120,15 @@ class ClockSampler:
             self.p.kill()
         self.f.flush()
         self.f.seek(0)
-        sm, reasons, smax, pw = [], set(), None, []
+        rows, reasons, smax = [], set(), None
         names = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
         for line in self.f.read().splitlines():
             parts = [x.strip() for x in line.split(",")]
             if len(parts) < 7:
                 continue
             try:
-                sm.append(float(parts[0]))
+                rows.append((float(parts[0]), float(parts[2])))
                 smax = float(parts[1])
-                pw.append(float(parts[2]))
             except ValueError:
                 continue
             for n, v in zip(names, parts[3:7]):
@@ -121,13 +138,15 @@ class ClockSampler:
             os.unlink(self.f.name)
         except OSError:
             pass
-        if sm:
-            sm.sort()
-            # median of the upper half = clocks under load (idle samples before/after are low)
-            hi = sm[len(sm) // 2:]
-            out["sm_mhz"] = hi[len(hi) // 2]
-            out["samples"] = len(sm)
-            out["power_w_max"] = max(pw) if pw else None
+        if rows:
+            # samples under load: power above the midpoint between the idle floor and the peak of this run
+            pw = [r[1] for r in rows]
+            thr = min(pw) + 0.5 * (max(pw) - min(pw))
+            load = sorted(r[0] for r in rows if r[1] >= thr) or sorted(r[0] for r in rows)
+            out["sm_mhz"] = load[len(load) // 2]
+            out["samples"] = len(rows)
+            out["samples_under_load"] = len(load)
+            out["power_w_max"] = max(pw)
         out["sm_max_mhz"] = smax
         out["reasons"] = sorted(reasons)
         return out
@@ -143,9 +162,20 @@ def time_oracle(L, U_real, iters: int):
     return time.perf_counter() - t0, oracle.threads()
 
 
+def lattice_name(L) -> str:
+    return "x".join(map(str, L))
+
+
+def workload_name(L, prec: str, stor: int, plaq_target: float) -> str:
+    """`config.workload`, the same string in both arms (the reference arm times the fp64 oracle on the same field)."""
+    return (f"configs[2]-shaped: {lattice_name(L)} SU(3), {prec}, {stor}-real, rough links plaquette {plaq_target} "
+            f"+ Haar gauge transform, alpha {ALPHA}")
+
+
 def run_reference(args, L):
-    """--impl reference: the oracle (unmodified, as it stands) on the box's host cores, same
-    config / metric / unit; each step = one oracle iteration on the same 32^4-shaped workload."""
+    """--impl reference: the oracle (unmodified, as it stands) on the box's host cores, same config / metric / unit as
+    the CUDA arm; each step = one full oracle iteration of the same lattice (about 1 s at 32^4 on 16 threads), W warm-up
+    and K timed steps as asked, capped at 60 iterations in total so that the run ends within a few minutes."""
     rank = int(os.environ.get("RANK", "0"))
     if rank != 0:
         return
@@ -155,10 +185,11 @@ def run_reference(args, L):
     dev = "cuda" if torch.cuda.is_available() else "cpu"
     U = gi.make_config(L, gi.CONFIG_SEED + 2, args.plaquette, device=dev).cpu()
     Ur = gi.as_real(U)
-    steps = max(1, min(args.steps, 3))         # bounded sample: a few iterations of the full lattice
-    warm = min(args.warmup, 1)
+    per_iter_cap = 60 if V <= (1 << 20) else 4
+    steps = max(1, min(args.steps, per_iter_cap))
+    warm = max(0, min(args.warmup, per_iter_cap - steps, 5))
     if warm:
-        time_oracle(L, Ur, 1)
+        time_oracle(L, Ur, warm)
     sec, thr = time_oracle(L, Ur, steps)
     # oracle.iterate does 1 initial measurement + steps x (update + measurement)
     val = steps / sec
@@ -166,14 +197,17 @@ def run_reference(args, L):
         "impl": "reference", "metric": "gauge_fix_iterations_per_s", "value": val, "unit": "iterations/s",
         "n_gpus": args.gpus, "steps": steps, "warmup": warm, "ms_per_step": 1e3 * sec / steps,
         "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
-        "config": {"workload": f"{'x'.join(map(str, L))} SU(3), plaquette {args.plaquette}, alpha {ALPHA}",
-                   "sites": V, "note": "oracle/lgf_oracle.cpp (plain C++, OpenMP over sites/lines) on host cores"},
+        "config": {"workload": workload_name(L, args.precision, args.storage, args.plaquette), "sites": V,
+                   "note": "oracle/lgf_oracle.cpp (plain C++, fp64, full 3x3 links, OpenMP over sites/lines) on host cores"},
         "cpu_baseline": {"value": val, "unit": "iterations/s", "cores": thr, "kind": "oracle",
-                         "sample": f"{steps} full iterations of the {'x'.join(map(str, L))} lattice"},
+                         "sample": f"{steps} full iterations of the {lattice_name(L)} lattice"},
         "e2e": {"value": val, "unit": "iterations/s", "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
         "gpu_launches": 0,
     }
     print(json.dumps(line), flush=True)
+
+
+ALL_MODES = [("f64", 18), ("f64", 12), ("f32", 18), ("f32", 12)]
 
 
 def main():
@@ -199,72 +233,89 @@ def main():
     if world > 1:
         dist.init_process_group("nccl", device_id=dev)
 
-    V = gi.volume(L)
     K, W = args.steps, max(args.warmup, 3)
     peak, peak_src = measured_peak()
-
-    # every rank: its own seeded lattice (replicas only)
-    U = gi.make_config(L, replicas.rank_seed(gi.CONFIG_SEED + 2, rank), args.plaquette, device=dev)
-    plaq = gi.mean_plaquette(U, L)
-
-    primary = (args.precision, args.storage)
-    modes = [primary]
-    if args.modes == "all":
-        modes += [m for m in [("f64", 18), ("f64", 12), ("f32", 18), ("f32", 12)] if m != primary]
 
     def barrier():
         if world > 1:
             dist.barrier()
         torch.cuda.synchronize()
 
-    results = {}
-    clocks = None
-    total_launches = 0
-    for (prec, stor) in modes:
-        dt = torch.float64 if prec == "f64" else torch.float32
-        gf = lgf.GaugeFixer(L, lgf.LGF_F64 if prec == "f64" else lgf.LGF_F32, stor, device=str(dev))
-        Ud = gi.as_real(U, dt)                       # device tensor: inputs resident in HBM
-        gf.load(Ud)
-        del Ud
-        gf.iterate(W, ALPHA)                         # warm-up (also captures the graph)
-        stream = torch.cuda.current_stream(dev)
-        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
-        sampler = ClockSampler(local) if (prec, stor) == primary and rank == 0 else None
-        barrier()
-        n0 = gf.launch_count()
-        e0.record(stream)
-        gf.iterate_async(K, ALPHA)
-        e1.record(stream)
-        res = gf.wait()
-        barrier()
-        launches = gf.launch_count() - n0
-        ms = e0.elapsed_time(e1)
-        if sampler:
-            clocks = sampler.stop()
-        ms = replicas.max_over_ranks(ms, dev)
-        kern_ms, _ = gf.profile_iterate(20, ALPHA)
-        w = 8 if prec == "f64" else 4
-        b_iter = (12 * stor + 64) * w
-        kernels = {}
-        for k, t_ms in kern_ms.items():
-            b = bytes_per_site(k, stor, w) * V
-            kernels[k] = {"ms": t_ms, "algorithmic_GBps": b / (t_ms * 1e-3) / 1e9,
-                          "frac_of_peak": b / (t_ms * 1e-3) / 1e9 / peak,
-                          "share_of_iteration": t_ms / sum(kern_ms.values())}
-        results[(prec, stor)] = {
-            "iterations_per_s": world * K / (ms * 1e-3), "ms_per_iteration": ms / K,
-            "site_updates_per_s": world * K * V / (ms * 1e-3),
-            "algorithmic_GBps": b_iter * V * K / (ms * 1e-3) / 1e9,
-            "frac_of_hbm_peak": b_iter * V * K / (ms * 1e-3) / 1e9 / peak,
-            "frac_of_nominal_8TBps": b_iter * V * K / (ms * 1e-3) / 1e9 / 8000.0,   # north_star's nominal figure
-            "bytes_per_site_iteration": b_iter, "theta": res.theta, "F": res.F,
-            "launches": launches, "kernels": kernels,
-        }
-        if (prec, stor) == primary:
-            total_launches = launches
-        gf.close()
-        del gf
-        torch.cuda.empty_cache()
+    def time_modes(Lx, U, modes, K_, W_, hold_primary_s=0.0):
+        """Time K_ graph-replayed iterations (after W_ warm-up iterations) of lattice Lx in every mode of `modes`, then the
+        per-kernel split.  Inputs are resident in HBM before the timed region.  Returns {(prec, stor): result}."""
+        Vx = gi.volume(Lx)
+        lkey = lattice_name(Lx)
+        out = {}
+        for i, (prec, stor) in enumerate(modes):
+            dt = torch.float64 if prec == "f64" else torch.float32
+            gf = lgf.GaugeFixer(Lx, lgf.LGF_F64 if prec == "f64" else lgf.LGF_F32, stor, device=str(dev))
+            Ud = gi.as_real(U, dt)                       # device tensor: inputs resident in HBM
+            gf.load(Ud)
+            del Ud
+            gf.iterate(W_, ALPHA)                        # warm-up (also captures the graph)
+            stream = torch.cuda.current_stream(dev)
+            e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            barrier()
+            n0 = gf.launch_count()
+            e0.record(stream)
+            gf.iterate_async(K_, ALPHA)
+            e1.record(stream)
+            res = gf.wait()
+            barrier()
+            launches = gf.launch_count() - n0
+            ms = replicas.max_over_ranks(e0.elapsed_time(e1), dev)
+            if i == 0 and hold_primary_s > 0:
+                # keep the same kernels running (untimed) so that the 50 ms clock sampler sees them under load
+                t_end = time.perf_counter() + hold_primary_s
+                while time.perf_counter() < t_end:
+                    gf.iterate(max(K_, 50), ALPHA)
+            kern_ms, _ = gf.profile_iterate(20, ALPHA)
+            info = gf.path_info()
+            w = 8 if prec == "f64" else 4
+            b_iter = (12 * stor + 64) * w
+            kernels = {}
+            for k, t_ms in kern_ms.items():
+                b = bytes_per_site(k, stor, w) * Vx
+                frac = b / (t_ms * 1e-3) / 1e9 / peak
+                kernels[k] = {"ms": t_ms, "algorithmic_GBps": b / (t_ms * 1e-3) / 1e9, "frac_of_peak": frac,
+                              "share_of_iteration": t_ms / sum(kern_ms.values())}
+                dram, src = ncu_traffic(lkey, f"{prec}_{stor}", k)
+                if dram is not None:
+                    # what the kernel really pulled through HBM under ncu (cold L2) over the live time: an upper bound of
+                    # its HBM rate inside the pipeline, where Delta-sized fields may be L2-resident (SURVEY.md §8(d) caveat)
+                    kernels[k]["ncu_dram_bytes"] = dram
+                    kernels[k]["ncu_dram_GBps"] = dram / (t_ms * 1e-3) / 1e9
+                    kernels[k]["ncu_source"] = src
+                if frac > 1.0:
+                    kernels[k]["note"] = "above the copy peak: part of this kernel's algorithmic bytes are served by the L2"
+            out[(prec, stor)] = {
+                "iterations_per_s": world * K_ / (ms * 1e-3), "ms_per_iteration": ms / K_,
+                "site_updates_per_s": world * K_ * Vx / (ms * 1e-3),
+                "algorithmic_GBps": b_iter * Vx * K_ / (ms * 1e-3) / 1e9,
+                "frac_of_hbm_peak": b_iter * Vx * K_ / (ms * 1e-3) / 1e9 / peak,
+                "frac_of_nominal_8TBps": b_iter * Vx * K_ / (ms * 1e-3) / 1e9 / 8000.0,   # north_star's nominal figure
+                "bytes_per_site_iteration": b_iter, "theta": res.theta, "F": res.F, "steps": K_,
+                "launches": launches, "fft_path": info["fft_path"], "fused_update": info["fused"],
+                "kernels_below_0.70_of_peak": sorted(k for k, v in kernels.items() if v["frac_of_peak"] < 0.70),
+                "kernels": kernels,
+            }
+            gf.close()
+            del gf
+            torch.cuda.empty_cache()
+        return out
+
+    # every rank: its own seeded lattice (replicas only)
+    V = gi.volume(L)
+    U = gi.make_config(L, replicas.rank_seed(gi.CONFIG_SEED + 2, rank), args.plaquette, device=dev)
+    plaq = gi.mean_plaquette(U, L)
+    primary = (args.precision, args.storage)
+    modes = [primary] + ([m for m in ALL_MODES if m != primary] if args.modes == "all" else [])
+
+    sampler = ClockSampler(local) if rank == 0 else None
+    t_load0 = time.perf_counter()
+    results = time_modes(L, U, modes, K, W, hold_primary_s=ClockSampler.kMinLoadSeconds if rank == 0 or world > 1 else 0.0)
+    total_launches = results[primary]["launches"]
 
     # ---- e2e: the user's call sequence with HOST buffers: load (H2D) + fix/iterate + store (D2H) ----
     e2e = None
@@ -296,27 +347,43 @@ def main():
         gf.close()
         del gf, host_in, host_out
 
+    # ---- the other headline lattices (configs[3], configs[4]); rank 0's clocks keep being sampled ----
+    lattices = {}
+    if args.lattices != "none":
+        for spec in args.lattices.split(";"):
+            Lx = tuple(int(x) for x in spec.split(","))
+            if Lx == L:
+                continue
+            idx = 3 if Lx == (48, 48, 48, 8) else 4
+            Ux = gi.make_config(Lx, replicas.rank_seed(gi.CONFIG_SEED + idx, rank), 0.58 if idx == 3 else 0.59, device=dev)
+            rx = time_modes(Lx, Ux, ALL_MODES, args.lattice_steps, 3)
+            del Ux
+            torch.cuda.empty_cache()
+            lattices[lattice_name(Lx)] = {"sites": gi.volume(Lx), "steps": args.lattice_steps, "warmup": 3,
+                                          "modes": {f"{p}_{s}": r for (p, s), r in rx.items()}}
+    clocks = sampler.stop() if sampler else None
+
     # ---- CPU baseline: the oracle, bounded sample, rank 0 at N = 1 only ----
     cpu = None
     if rank == 0 and world == 1 and not args.no_cpu_baseline:
         iters = 3 if V <= (1 << 20) else 1
         sec, thr = time_oracle(L, gi.as_real(U).cpu(), iters)
         cpu = {"value": iters / sec, "unit": "iterations/s", "cores": thr, "kind": "oracle",
-               "sample": f"{iters} full iterations of the same {'x'.join(map(str, L))} lattice ({sec:.1f} s)"}
+               "sample": f"{iters} full iterations of the same {lattice_name(L)} lattice ({sec:.1f} s)"}
 
     if rank == 0:
         pr = results[primary]
         dom = max(pr["kernels"].items(), key=lambda kv: kv[1]["ms"])
         w = 8 if primary[0] == "f64" else 4
         dom_bytes = bytes_per_site(dom[0], primary[1], w) * V
-        mode_key = f"{primary[0]}_{primary[1]}"
+        traffic, traffic_src = ncu_traffic(lattice_name(L), f"{primary[0]}_{primary[1]}", dom[0])
         line = {
             "metric": "gauge_fix_iterations_per_s", "value": pr["iterations_per_s"], "unit": "iterations/s",
             "n_gpus": world, "steps": K, "warmup": W, "ms_per_step": pr["ms_per_iteration"],
             "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
             "dtype": primary[0], "data": "synthetic",
-            "config": {"workload": f"configs[2]-shaped: {'x'.join(map(str, L))} SU(3), {primary[0]}, {primary[1]}-real, "
-                                   f"rough links plaquette {plaq:.4f} + Haar gauge transform, alpha {ALPHA}",
+            "config": {"workload": workload_name(L, primary[0], primary[1], args.plaquette),
+                       "measured_plaquette": plaq,
                        "sites": V, "parallelism": "replicas only" if world > 1 else "1 GPU",
                        "l2": "inputs larger than L2 (links %.0f MB > 126 MB)" % (4 * primary[1] * V * w / 1e6),
                        "hbm_peak_GBps": peak, "hbm_peak_source": peak_src},
@@ -325,13 +392,14 @@ def main():
             "iteration_frac_of_hbm_roofline": pr["frac_of_hbm_peak"],
             "iteration_frac_of_nominal_8TBps": pr["frac_of_nominal_8TBps"],
             "roofline": {"bound": "hbm", "kernel": dom[0], "achieved": dom[1]["algorithmic_GBps"], "peak": peak,
-                         "unit": "GB/s", "frac": dom[1]["frac_of_peak"], "traffic": ncu_traffic(mode_key, dom[0]),
+                         "unit": "GB/s", "frac": dom[1]["frac_of_peak"], "traffic": traffic, "traffic_source": traffic_src,
                          "algorithmic_bytes_per_launch": dom_bytes, "peak_source": peak_src},
             "cpu_baseline": cpu,
             "e2e": e2e,
             "gpu_launches": total_launches,
             "clocks": clocks,
             "modes": {f"{p}_{s}": {k: v for k, v in r.items()} for (p, s), r in results.items()},
+            "lattices": lattices,
         }
         print(json.dumps(line), flush=True)
     if world > 1:

@@ -271,6 +271,35 @@ def test_rough_config_F_monotone_and_counts():
     assert thh[20] < 1e-3
 
 
+def test_fix_count_semantics():
+    """Reading #12: strict theta < tol tested after each update on the updated links;
+    `iterations` = number of updates applied; a field already below tolerance takes 0 updates; max_iter caps."""
+    L = (4, 6, 3, 2)
+    U = gi.make_config(L, 20, 0.59)
+    tol = 1e-8
+    _, n, theta, F, thh, Fh = oracle.fix(L, U, ALPHA, tol, 5000)
+    assert len(thh) == n + 1 and len(Fh) == n + 1 and n >= 2
+    assert thh[n] < tol <= thh[n - 1]                   # first crossing, strict
+    assert np.all(thh[:n] >= tol)                       # no earlier iterate was already below
+    assert theta == thh[n] and F == Fh[n]
+    # the history is the trajectory of `iterate`: same updates, nothing skipped or repeated
+    ref, thi, Fi = oracle.iterate(L, U, n, ALPHA)
+    assert np.array_equal(thi, thh) and np.array_equal(Fi, Fh)
+    # strictness: a tolerance equal to a value on the trajectory does not stop there
+    _, n_eq, _, _, _, _ = oracle.fix(L, U, ALPHA, float(thh[n - 1]), 5000)
+    assert n_eq == n                                    # theta[n-1] == tol continues, theta[n] < tol stops
+    _, n_eq2, _, _, _, _ = oracle.fix(L, U, ALPHA, float(thh[n]), 5000)
+    assert n_eq2 > n                                    # theta == tol is NOT converged
+    # max_iter caps the count; the result is the k-th iterate
+    for k in (0, 1, 3):
+        out, nk, thk, Fk, hk, _ = oracle.fix(L, U, ALPHA, 1e-300, k)
+        assert nk == k and len(hk) == k + 1 and thk == thh[k]
+    # already below tolerance: zero updates, links untouched
+    out, n0, th0, _, h0, _ = oracle.fix(L, U, ALPHA, 1e30, 5000)
+    assert n0 == 0 and th0 == thh[0] and len(h0) == 1
+    assert np.array_equal(out, gi.from_real(gi.as_real(U)).numpy().reshape(out.shape))
+
+
 # ---------------------------------------------------------------- P11: brute-force convolution
 def test_fourier_acceleration_equals_position_space_convolution():
     L = (4, 4, 2, 2)
