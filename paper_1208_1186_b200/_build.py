@@ -8,8 +8,13 @@ _HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(_HERE, "csrc")
 LIB = os.path.join(_HERE, "liblgf.so")
 SOURCES = ["lgf_api.cu", "lgf_fft_inst.cu", "lgf_fft_inst_f64.cu", "lgf_fft_inst_f32.cu", "lgf_fft_pipe_f64.cu", "lgf_fft_pipe_f32.cu"]
-HEADERS = ["lgf_math.cuh", "lgf_site.cuh", "lgf_site_mu.cuh", "lgf_fft.cuh", "lgf_regfft.cuh", "lgf_fft_ct.cuh", "lgf_fft_inst.cuh",
-           "lgf_fft_inst_impl.cuh", "lgf_async.cuh", "lgf_fft_pipe.cuh", "lgf_fft_pipe_inst.cuh", "lgf_fft_pipe_inst_impl.cuh", os.path.join("..", "..", "include", "lgf.h")]
+
+
+def _headers() -> list:
+    """Every header a translation unit may include: all of csrc/*.cuh plus the public C header."""
+    import glob
+    return sorted(glob.glob(os.path.join(CSRC, "*.cuh"))) + [os.path.join(_HERE, "..", "include", "lgf.h")]
+
 
 NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo", "-O3", "-std=c++17", "-Xcompiler", "-fPIC"]
 LINK_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-shared", "--cudart", "shared"]
@@ -19,7 +24,7 @@ def _stale() -> bool:
     if not os.path.exists(LIB):
         return True
     t = os.path.getmtime(LIB)
-    files = [os.path.join(CSRC, f) for f in SOURCES + HEADERS] + [os.path.abspath(__file__)]
+    files = [os.path.join(CSRC, f) for f in SOURCES] + _headers() + [os.path.abspath(__file__)]
     return any(os.path.getmtime(f) > t for f in files)
 
 

@@ -4,6 +4,8 @@
 // entry point launches kernels and reports LGF_ECUDA if that fails.
 #include "../../include/lgf.h"
 
+#include <cuda.h>
+
 #include <cmath>
 #include <cstdio>
 #include <cstdlib>
@@ -172,6 +174,7 @@ struct lgf_ctx {
     const ZtPipeEntry* zt_pipe;
     XyPipeArgs xyp_args;
     int xyp_grid, ztp_grid;
+    alignas(64) CUtensorMap zt_omap;     // output tensor (Delta~, natural layout) of a K3 that stores through the TMA unit
     // fused K5+K1 marching kernel (lgf_site_fused.cuh); -1: not used
     int fused_tile;
     MarchGeom mgeom;
@@ -361,6 +364,9 @@ bool plan_passes(lgf_ctx* c) {
         while ((1 << sh) < c->zt_pipe->cx) ++sh;
         P.cxb_shift = sh;
         P.chunks_per_comp = (int)(LxLy >> sh);
+        P.perm_c = c->zt_pipe->perm_c;
+        P.perm_d = c->zt_pipe->perm_d;
+        P.perm_lq = c->zt_pipe->tstore ? c->zt_pipe->perm_d / 4 : c->zt_pipe->perm_d;
     }
     if (c->zt_ct || c->zt_pipe) {
         ZtArgs& A = c->zt_args;
@@ -378,6 +384,36 @@ bool plan_passes(lgf_ctx* c) {
         A.y_n2 = L[1] / A.y_n1;
     }
     return true;
+}
+
+// CUtensorMap of the natural-layout Delta~ field D[c][t][z][y][x] as the 5-D tensor (2 reals * xy, z, t mod D, t div D, c)
+// for a K3 that stores whole quarter tiles through the TMA unit (fft_zt_pipe3q): box = (2 CX reals, Nz + 1, D/4, C, 1),
+// whose (Nz+1)-th z entry (the pad of the shared-memory rows) falls outside the tensor and is clipped by the hardware.
+int make_zt_output_map(lgf_ctx* c) {
+    const ZtPipeEntry* e = c->zt_pipe;
+    if (!e || !e->tstore) return LGF_OK;
+    typedef CUresult (*EncodeFn)(CUtensorMap*, CUtensorMapDataType, cuuint32_t, void*, const cuuint64_t*, const cuuint64_t*,
+                                 const cuuint32_t*, const cuuint32_t*, CUtensorMapInterleave, CUtensorMapSwizzle,
+                                 CUtensorMapL2promotion, CUtensorMapFloatOOBfill);
+    void* fn = nullptr;
+    cudaDriverEntryPointQueryResult qres;
+    CU(cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &fn, cudaEnableDefault, &qres));
+    if (!fn || qres != cudaDriverEntryPointSuccess) return cuda_fail(cudaErrorNotSupported, "cuTensorMapEncodeTiled entry point");
+    const cuuint64_t cb = 2 * c->wbytes, LxLy = (cuuint64_t)c->L[0] * c->L[1], Nz = c->L[2];
+    const cuuint64_t C = e->perm_c, D = e->perm_d;
+    const cuuint64_t dims[5] = {2 * LxLy, Nz, D, C, 4};
+    const cuuint64_t strides[4] = {LxLy * cb, LxLy * Nz * cb, D * LxLy * Nz * cb, (cuuint64_t)c->V * cb};
+    const cuuint32_t box[5] = {(cuuint32_t)(2 * e->cx), (cuuint32_t)(Nz + 1), (cuuint32_t)(D / 4), (cuuint32_t)C, 1};
+    const cuuint32_t estr[5] = {1, 1, 1, 1, 1};
+    const CUresult r = reinterpret_cast<EncodeFn>(fn)(
+        &c->zt_omap, c->precision == LGF_F64 ? CU_TENSOR_MAP_DATA_TYPE_FLOAT64 : CU_TENSOR_MAP_DATA_TYPE_FLOAT32, 5,
+        c->ws + c->lo.delta, dims, strides, box, estr, CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_NONE,
+        CU_TENSOR_MAP_L2_PROMOTION_NONE, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
+    if (r != CUDA_SUCCESS) {
+        snprintf(g_last_error, sizeof(g_last_error), "cuTensorMapEncodeTiled failed with CUresult %d", (int)r);
+        return LGF_ECUDA;
+    }
+    return LGF_OK;
 }
 
 template <typename T>
@@ -564,7 +600,7 @@ struct Impl {
             Cx<T>* d2 = reinterpret_cast<Cx<T>*>(c->ws + c->lo.delta2);
             if (k == 1) {
                 const ZtPipeEntry* e = c->zt_pipe;
-                void* args[] = {&d2, &dptr, &c->zt_args, &done};          // layout B -> natural
+                void* args[] = {&d2, &dptr, &c->zt_args, &done, &c->zt_omap};          // layout B -> natural (fifth: tstore kernels only)
                 CU(launch_exc(c, e->kernel, dim3(c->ztp_grid), dim3(e->threads), args, e->smem));
             } else {
                 const XyPipeEntry* e = k == 0 ? c->xy_pipe : c->xy_pipe_inv;
@@ -625,6 +661,10 @@ struct Impl {
         }
         {
             const int rc = plan_fused(c);
+            if (rc) return rc;
+        }
+        {
+            const int rc = make_zt_output_map(c);
             if (rc) return rc;
         }
         return upload_tables<T>(c);

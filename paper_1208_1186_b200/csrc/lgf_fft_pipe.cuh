@@ -53,6 +53,10 @@ struct XyPipeArgs {
     int chunks_per_comp;    // Lx * Ly >> cxb_shift
     int pt;                 // layout-B t pitch in elements: CX * (Lz + 1)
     int tile_elems;         // layout-B tile size in elements: pt * Lt
+    // order of the t rows inside a layout-B tile: with t = n2 + perm_d * m (n2 < perm_d, m < perm_c) and n2 = perm_lq * q + l,
+    // row rho(t) = (q * perm_c + m) * perm_lq + l.  perm_c = 1, perm_d = perm_lq = Lt is the natural order; the quarter-ring
+    // K3 of lgf_fft_pipe3.cuh asks for the (C, D) split of its t lines with perm_lq = D / 4.
+    int perm_c, perm_d, perm_lq;
 };
 
 // Shared-memory planes are dense (one bulk copy per tile); bank conflicts of the passes that walk
@@ -176,7 +180,9 @@ fft_xy_pipe(const Cx<T>* in, Cx<T>* out, const XyPipeArgs A, const int* done) {
                 const int gp = plane0 + pl;
                 const int comp = gp / A.planes_per_comp, zt = gp - comp * A.planes_per_comp;
                 const int t = zt / A.nz, z = zt - t * A.nz;
-                Cx<T>* dbase = out + (size_t)comp * A.chunks_per_comp * A.tile_elems + (size_t)t * A.pt + ((size_t)z << A.cxb_shift);
+                const int tm = t / A.perm_d, tn = t - tm * A.perm_d, tq = tn / A.perm_lq;
+                const int rho = (tq * A.perm_c + tm) * A.perm_lq + (tn - tq * A.perm_lq);
+                Cx<T>* dbase = out + (size_t)comp * A.chunks_per_comp * A.tile_elems + (size_t)rho * A.pt + ((size_t)z << A.cxb_shift);
                 const Cx<T>* sp = tile + pl * PLANE;
 #pragma unroll 4
                 for (int q = gtid; q < PLANE; q += GT) {

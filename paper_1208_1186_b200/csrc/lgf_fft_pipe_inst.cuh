@@ -25,6 +25,9 @@ struct ZtPipeEntry {
     int nbuf;
     size_t smem;
     const void* kernel;      // fft_zt_pipe<...>  layout B -> natural
+    // quarter-ring kernel (fft_zt_pipe3q): layout B holds the t rows quarter by quarter (XyPipeArgs::perm_*; perm_c x perm_d = its split of the t lines),
+    // and the kernel takes a fifth argument, the CUtensorMap of its output (tstore = 1); 0, 1, nt otherwise
+    int tstore, perm_c, perm_d;
 };
 
 // precision: 0 = float, 1 = double; LGF_XYP_VARIANT / LGF_ZTP_VARIANT pick the v-th match (A/B knob)

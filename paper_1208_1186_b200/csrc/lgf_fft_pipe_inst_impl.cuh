@@ -1,6 +1,7 @@
 // lgf_fft_pipe_inst_impl.cuh -- entry builders shared by the two instantiation units.
 #pragma once
 #include "lgf_fft_pipe.cuh"
+#include "lgf_fft_pipe3.cuh"
 #include "lgf_fft_pipe_inst.cuh"
 
 namespace lgf {
@@ -27,7 +28,7 @@ struct ZtP {
     static_assert(kSmem <= 227 * 1024, "tile ring exceeds shared memory");
     static_assert((CX & (CX - 1)) == 0, "CX must be a power of two");
     static ZtPipeEntry entry() {
-        return ZtPipeEntry{NZ, NT, CX, GT * NG, NBUF, kSmem, (const void*)&fft_zt_pipe<T, SZ, ST_, CX, GT, NG, NBUF>};
+        return ZtPipeEntry{NZ, NT, CX, GT * NG, NBUF, kSmem, (const void*)&fft_zt_pipe<T, SZ, ST_, CX, GT, NG, NBUF>, 0, 1, NT};
     }
 };
 
@@ -40,7 +41,44 @@ struct ZtPH {
     static_assert(kSmem <= 227 * 1024, "half-tile ring exceeds shared memory");
     static_assert((CX & (CX - 1)) == 0, "CX must be a power of two");
     static ZtPipeEntry entry() {
-        return ZtPipeEntry{NZ, NT, CX, GT, 3, kSmem, (const void*)&fft_zt_pipe_halves<T, SZ, ST_, CX, GT>};
+        return ZtPipeEntry{NZ, NT, CX, GT, 3, kSmem, (const void*)&fft_zt_pipe_halves<T, SZ, ST_, CX, GT>, 0, 1, NT};
+    }
+};
+
+// three-register-stage K3 (lgf_fft_pipe3.cuh): ring of whole tiles / half-tile ring
+template <typename T, int NZ, int Z1, int NT, int T1, int CX, int GT, int NG, int NBUF>
+struct ZtP3 {
+    typedef LineSplit<NZ, Z1> SZ;
+    typedef LineSplit<NT, T1> ST_;
+    static constexpr size_t kSmem = sizeof(Cx<T>) * (size_t)NBUF * CX * (NZ + 1) * NT + 8 * NBUF;
+    static_assert(kSmem <= 227 * 1024, "tile ring exceeds shared memory");
+    static_assert((CX & (CX - 1)) == 0, "CX must be a power of two");
+    static ZtPipeEntry entry() {
+        return ZtPipeEntry{NZ, NT, CX, GT * NG, NBUF, kSmem, (const void*)&fft_zt_pipe3<T, SZ, ST_, CX, GT, NG, NBUF>, 0, 1, NT};
+    }
+};
+template <typename T, int NZ, int Z1, int NT, int T1, int CX, int GT>
+struct ZtP3H {
+    typedef LineSplit<NZ, Z1> SZ;
+    typedef LineSplit<NT, T1> ST_;
+    static constexpr size_t kSmem = sizeof(Cx<T>) * (size_t)3 * CX * (NZ + 1) * (NT / 2) + 8 * 3;
+    static_assert(kSmem <= 227 * 1024, "half-tile ring exceeds shared memory");
+    static_assert((CX & (CX - 1)) == 0, "CX must be a power of two");
+    static ZtPipeEntry entry() {
+        return ZtPipeEntry{NZ, NT, CX, GT, 3, kSmem, (const void*)&fft_zt_pipe3_halves<T, SZ, ST_, CX, GT>, 0, 1, NT};
+    }
+};
+
+// quarter ring + TMA tensor store (fft_zt_pipe3q)
+template <typename T, int NZ, int Z1, int NT, int T1, int CX, int GT>
+struct ZtP3Q {
+    typedef LineSplit<NZ, Z1> SZ;
+    typedef LineSplit<NT, T1> ST_;
+    static constexpr size_t kSmem = sizeof(Cx<T>) * ((size_t)6 * CX * (NZ + 1) * (NT / 4) + (size_t)(NT / T1) * (T1 - 1)) + 8 * 6;
+    static_assert(kSmem <= 227 * 1024, "quarter-tile ring exceeds shared memory");
+    static_assert((CX & (CX - 1)) == 0, "CX must be a power of two");
+    static ZtPipeEntry entry() {
+        return ZtPipeEntry{NZ, NT, CX, GT, 6, kSmem, (const void*)&fft_zt_pipe3q<T, SZ, ST_, CX, GT>, 1, T1, NT / T1};
     }
 };
 
