@@ -174,7 +174,8 @@ struct lgf_ctx {
     const ZtPipeEntry* zt_pipe;
     XyPipeArgs xyp_args;
     int xyp_grid, ztp_grid;
-    alignas(64) CUtensorMap zt_omap;     // output tensor (Delta~, natural layout) of a K3 that stores through the TMA unit
+    alignas(64) CUtensorMap zt_omap;     // fft_zt_pipe3q's output tensor (Delta~, natural layout), stored through the TMA unit
+    alignas(64) CUtensorMap xy_bmap;     // fft_xy_pipe_io's output tensor (the layout-B spectrum)
     // fused K5+K1 marching kernel (lgf_site_fused.cuh); -1: not used
     int fused_tile;
     MarchGeom mgeom;
@@ -366,7 +367,12 @@ bool plan_passes(lgf_ctx* c) {
         P.chunks_per_comp = (int)(LxLy >> sh);
         P.perm_c = c->zt_pipe->perm_c;
         P.perm_d = c->zt_pipe->perm_d;
-        P.perm_lq = c->zt_pipe->tstore ? c->zt_pipe->perm_d / 4 : c->zt_pipe->perm_d;
+        P.perm_lq = c->zt_pipe->tstore == 1 ? c->zt_pipe->perm_d / 4 : c->zt_pipe->perm_d;
+        // K2 stores a plane as boxes of `store_tiles` layout-B tiles x CX sites (a tensor-map box extent is at most 256)
+        int st = P.chunks_per_comp < 256 ? P.chunks_per_comp : 256;
+        while (P.chunks_per_comp % st) --st;
+        P.store_tiles = st;
+        P.nstores = P.chunks_per_comp / st;
     }
     if (c->zt_ct || c->zt_pipe) {
         ZtArgs& A = c->zt_args;
@@ -386,32 +392,51 @@ bool plan_passes(lgf_ctx* c) {
     return true;
 }
 
-// CUtensorMap of the natural-layout Delta~ field D[c][t][z][y][x] as the 5-D tensor (2 reals * xy, z, t mod D, t div D, c)
-// for a K3 that stores whole quarter tiles through the TMA unit (fft_zt_pipe3q): box = (2 CX reals, Nz + 1, D/4, C, 1),
-// whose (Nz+1)-th z entry (the pad of the shared-memory rows) falls outside the tensor and is clipped by the hardware.
-int make_zt_output_map(lgf_ctx* c) {
-    const ZtPipeEntry* e = c->zt_pipe;
-    if (!e || !e->tstore) return LGF_OK;
-    typedef CUresult (*EncodeFn)(CUtensorMap*, CUtensorMapDataType, cuuint32_t, void*, const cuuint64_t*, const cuuint64_t*,
-                                 const cuuint32_t*, const cuuint32_t*, CUtensorMapInterleave, CUtensorMapSwizzle,
-                                 CUtensorMapL2promotion, CUtensorMapFloatOOBfill);
+typedef CUresult (*TensorMapEncodeFn)(CUtensorMap*, CUtensorMapDataType, cuuint32_t, void*, const cuuint64_t*, const cuuint64_t*,
+                                      const cuuint32_t*, const cuuint32_t*, CUtensorMapInterleave, CUtensorMapSwizzle,
+                                      CUtensorMapL2promotion, CUtensorMapFloatOOBfill);
+int encode_map(lgf_ctx* c, CUtensorMap* map, int rank, void* base, const cuuint64_t* dims, const cuuint64_t* strides,
+               const cuuint32_t* box) {
     void* fn = nullptr;
     cudaDriverEntryPointQueryResult qres;
     CU(cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &fn, cudaEnableDefault, &qres));
     if (!fn || qres != cudaDriverEntryPointSuccess) return cuda_fail(cudaErrorNotSupported, "cuTensorMapEncodeTiled entry point");
-    const cuuint64_t cb = 2 * c->wbytes, LxLy = (cuuint64_t)c->L[0] * c->L[1], Nz = c->L[2];
-    const cuuint64_t C = e->perm_c, D = e->perm_d;
-    const cuuint64_t dims[5] = {2 * LxLy, Nz, D, C, 4};
-    const cuuint64_t strides[4] = {LxLy * cb, LxLy * Nz * cb, D * LxLy * Nz * cb, (cuuint64_t)c->V * cb};
-    const cuuint32_t box[5] = {(cuuint32_t)(2 * e->cx), (cuuint32_t)(Nz + 1), (cuuint32_t)(D / 4), (cuuint32_t)C, 1};
     const cuuint32_t estr[5] = {1, 1, 1, 1, 1};
-    const CUresult r = reinterpret_cast<EncodeFn>(fn)(
-        &c->zt_omap, c->precision == LGF_F64 ? CU_TENSOR_MAP_DATA_TYPE_FLOAT64 : CU_TENSOR_MAP_DATA_TYPE_FLOAT32, 5,
-        c->ws + c->lo.delta, dims, strides, box, estr, CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_NONE,
-        CU_TENSOR_MAP_L2_PROMOTION_NONE, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
+    const CUresult r = reinterpret_cast<TensorMapEncodeFn>(fn)(
+        map, c->precision == LGF_F64 ? CU_TENSOR_MAP_DATA_TYPE_FLOAT64 : CU_TENSOR_MAP_DATA_TYPE_FLOAT32, (cuuint32_t)rank, base,
+        dims, strides, box, estr, CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_NONE, CU_TENSOR_MAP_L2_PROMOTION_NONE,
+        CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
     if (r != CUDA_SUCCESS) {
         snprintf(g_last_error, sizeof(g_last_error), "cuTensorMapEncodeTiled failed with CUresult %d", (int)r);
         return LGF_ECUDA;
+    }
+    return LGF_OK;
+}
+// The tensor maps of the kernels of the pipelined FFT path that store through the TMA unit.  Element = one real; a
+// complex number is two elements, so every box starts and ends on whole sites.
+//   fft_zt_pipe3q (K3, quarter tiles): the natural-layout Delta~ field D[c][t][z][y][x] as the 5-D tensor
+//   (2 xy, z, t mod D, t div D, c), box (2 CX, Nz + 1, D/4, C, 1).  The (Nz+1)-th z entry of a box -- the pad of the
+//   shared-memory rows -- falls outside the tensor and is clipped by the hardware.
+//   fft_xy_pipe_io (K2): layout B, D'[c][tile][row][z + pad][j], as the 4-D tensor (2 j, z, row, c * tiles + tile),
+//   box (2 CX, 1, 1, store_tiles).
+int make_pipe_maps(lgf_ctx* c) {
+    const ZtPipeEntry* e = c->zt_pipe;
+    if (!e || !c->xy_pipe) return LGF_OK;
+    const cuuint64_t cb = 2 * c->wbytes, LxLy = (cuuint64_t)c->L[0] * c->L[1], Nz = c->L[2], Nt = c->L[3];
+    if (e->tstore == 1) {
+        const cuuint64_t C = e->perm_c, D = e->perm_d;
+        const cuuint64_t dims[5] = {2 * LxLy, Nz, D, C, 4};
+        const cuuint64_t strides[4] = {LxLy * cb, LxLy * Nz * cb, D * LxLy * Nz * cb, (cuuint64_t)c->V * cb};
+        const cuuint32_t box[5] = {(cuuint32_t)(2 * e->cx), (cuuint32_t)(Nz + 1), (cuuint32_t)(D / 4), (cuuint32_t)C, 1};
+        const int rc = encode_map(c, &c->zt_omap, 5, c->ws + c->lo.delta, dims, strides, box);
+        if (rc) return rc;
+    }
+    if (c->xy_pipe->io) {
+        const XyPipeArgs& P = c->xyp_args;
+        const cuuint64_t dims[4] = {(cuuint64_t)(2 * e->cx), Nz + 1, Nt, (cuuint64_t)(4 * P.chunks_per_comp)};
+        const cuuint64_t strides[3] = {(cuuint64_t)e->cx * cb, (cuuint64_t)P.pt * cb, (cuuint64_t)P.tile_elems * cb};
+        const cuuint32_t box[4] = {(cuuint32_t)(2 * e->cx), 1, 1, (cuuint32_t)P.store_tiles};
+        return encode_map(c, &c->xy_bmap, 4, c->ws + c->lo.delta2, dims, strides, box);
     }
     return LGF_OK;
 }
@@ -600,13 +625,13 @@ struct Impl {
             Cx<T>* d2 = reinterpret_cast<Cx<T>*>(c->ws + c->lo.delta2);
             if (k == 1) {
                 const ZtPipeEntry* e = c->zt_pipe;
-                void* args[] = {&d2, &dptr, &c->zt_args, &done, &c->zt_omap};          // layout B -> natural (fifth: tstore kernels only)
+                void* args[] = {&d2, &dptr, &c->zt_args, &done, &c->zt_omap};          // layout B -> natural (fifth: fft_zt_pipe3q only)
                 CU(launch_exc(c, e->kernel, dim3(c->ztp_grid), dim3(e->threads), args, e->smem));
             } else {
                 const XyPipeEntry* e = k == 0 ? c->xy_pipe : c->xy_pipe_inv;
                 Cx<T>* inp = k == 0 ? delta_src(c) : dptr;                 // K2 reads Delta where K1 / K51 left it
                 Cx<T>* outp = k == 0 ? d2 : dptr;                          // K2: natural -> layout B; K4: in place
-                void* args[] = {&inp, &outp, &c->xyp_args, &done};
+                void* args[] = {&inp, &outp, &c->xyp_args, &done, &c->xy_bmap};      // (fifth: fft_xy_pipe_io only)
                 CU(launch_exc(c, k == 0 ? e->k_fwd : e->k_inv, dim3(k == 0 ? c->xyp_grid : c->xyp_inv_grid), dim3(e->threads), args, e->smem));
             }
             c->launches++;
@@ -664,7 +689,7 @@ struct Impl {
             if (rc) return rc;
         }
         {
-            const int rc = make_zt_output_map(c);
+            const int rc = make_pipe_maps(c);
             if (rc) return rc;
         }
         return upload_tables<T>(c);

@@ -67,12 +67,17 @@ const XyPipeEntry* find_xy_pipe_inv(int precision, int nx, int ny, const XyPipeE
     const char* e = getenv("LGF_XYP_INV_VARIANT");
     // measured: 48x48 fp32 planes run the inverse pass faster on 1-plane tiles (K4 24.9 -> 22.9 us at 48^3 x 8)
     int skip = e ? atoi(e) : ((precision == 0 && nx == 48 && ny == 48 && !getenv("LGF_XYP_VARIANT")) ? 1 : -1);
-    if (skip < 0) return fwd;
+    if (skip < 0 && fwd->k_inv) return fwd;
+    if (skip < 0) skip = 0;                        // a forward-only entry (fft_xy_pipe_io): the first entry that has an inverse kernel
     int n = 0;
     const XyPipeEntry* t = xyp_tab(precision, &n);
+    const XyPipeEntry* last = nullptr;
     for (int i = 0; i < n; ++i)
-        if (t[i].nx == nx && t[i].ny == ny && t[i].x_n1 == fwd->x_n1 && t[i].y_n1 == fwd->y_n1 && skip-- == 0) return &t[i];
-    return fwd;
+        if (t[i].nx == nx && t[i].ny == ny && t[i].x_n1 == fwd->x_n1 && t[i].y_n1 == fwd->y_n1 && t[i].k_inv) {
+            last = &t[i];
+            if (skip-- == 0) return last;
+        }
+    return last;
 }
 const XyPipeEntry* find_xy_pipe(int precision, int nx, int ny) {
     int n = 0, skip = variant("LGF_XYP_VARIANT");
@@ -101,7 +106,7 @@ cudaError_t prepare_pipe_kernels(int precision) {
     const XyPipeEntry* x = xyp_tab(precision, &n);
     for (int i = 0; i < n; ++i) {
         cudaError_t e = cudaFuncSetAttribute(x[i].k_fwd, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)x[i].smem);
-        if (e == cudaSuccess) e = cudaFuncSetAttribute(x[i].k_inv, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)x[i].smem);
+        if (e == cudaSuccess && x[i].k_inv) e = cudaFuncSetAttribute(x[i].k_inv, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)x[i].smem);
         if (e != cudaSuccess) return e;
     }
     const ZtPipeEntry* z = ztp_tab(precision, &n);

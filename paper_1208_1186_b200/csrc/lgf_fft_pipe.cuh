@@ -57,6 +57,7 @@ struct XyPipeArgs {
     // row rho(t) = (q * perm_c + m) * perm_lq + l.  perm_c = 1, perm_d = perm_lq = Lt is the natural order; the quarter-ring
     // K3 of lgf_fft_pipe3.cuh asks for the (C, D) split of its t lines with perm_lq = D / 4.
     int perm_c, perm_d, perm_lq;
+    int store_tiles, nstores;   // fft_xy_pipe_io's tensor stores: layout-B tiles per store (box extent, <= 256), stores per plane
 };
 
 // Shared-memory planes are dense (one bulk copy per tile); bank conflicts of the passes that walk
@@ -366,141 +367,6 @@ fft_zt_pipe(const Cx<T>* inB, Cx<T>* out, const ZtArgs A, const int* done) {
         fence_proxy_async();
         group_sync<GT, NG>(g);
         if (i + NBUF < my_tiles && gtid == 0) issue(i + NBUF);
-    }
-}
-
-// K3 for (z,t) planes too large for a ring of whole tiles (64 x 64 in fp64: 133 KB per tile): the
-// tile travels as two HALVES (t < NT/2, t >= NT/2; contiguous in layout B) through a ring of three
-// half-tile buffers.  Tile n's first half is fetched while tile n-1 is being transformed, its second
-// half while the z lines of the first half are transformed (z lines live inside one t row), so only
-// part of one half-tile fetch per tile is exposed.  One thread group (the whole CTA).
-template <typename T, class SZ, class ST_, int CX, int GT>
-__global__ void __launch_bounds__(GT, 1)
-fft_zt_pipe_halves(const Cx<T>* inB, Cx<T>* out, const ZtArgs A, const int* done) {
-    pdl_entry();
-    extern __shared__ __align__(128) unsigned char pipe_smem[];
-    if (done && *reinterpret_cast<const volatile int*>(done)) return;
-    constexpr int NZ = SZ::kN, NT = ST_::kN, PZ = CX, PT = CX * (NZ + 1), HT = NT / 2, HALF = PT * HT;
-    static_assert(NT % 2 == 0 && (HALF * sizeof(Cx<T>)) % 16 == 0 && GT % 32 == 0, "half tiles");
-    Cx<T>* bufs = reinterpret_cast<Cx<T>*>(pipe_smem);
-    uint64_t* full = reinterpret_cast<uint64_t*>(pipe_smem + sizeof(Cx<T>) * (size_t)3 * HALF);
-    const int tid = threadIdx.x;
-    const int ntiles = 4 * A.tiles_per_comp;
-    const int my_tiles = (int)blockIdx.x < ntiles ? (ntiles - (int)blockIdx.x + (int)gridDim.x - 1) / (int)gridDim.x : 0;
-    const long long gz = A.LxLy, gt = A.LxLy * NZ;
-    const Cx<T>* twz_f = reinterpret_cast<const Cx<T>*>(A.twz_fwd);
-    const Cx<T>* twz_i = reinterpret_cast<const Cx<T>*>(A.twz_inv);
-    const Cx<T>* twt_f = reinterpret_cast<const Cx<T>*>(A.twt_fwd);
-    const Cx<T>* twt_i = reinterpret_cast<const Cx<T>*>(A.twt_inv);
-
-    auto issue = [&](int k) {             // half k = 2 * (tile index of this CTA) + (0 | 1)
-        const int buf = k % 3;
-        const size_t id = (size_t)blockIdx.x + (size_t)(k >> 1) * gridDim.x;
-        const uint32_t bytes = (uint32_t)(HALF * sizeof(Cx<T>));
-        mbar_arrive_expect_tx(&full[buf], bytes);
-        bulk_g2s(bufs + (size_t)buf * HALF, inB + id * (size_t)(2 * HALF) + (size_t)(k & 1) * HALF, bytes, &full[buf]);
-    };
-    if (tid == 0) {
-        for (int b = 0; b < 3; ++b) mbar_init(&full[b], 1);
-        mbar_fence_init();
-        for (int k = 0; k < 3 && k < 2 * my_tiles; ++k) issue(k);
-    }
-    __syncthreads();
-
-    for (int i = 0; i < my_tiles; ++i) {
-        const int k0 = 2 * i, k1h = 2 * i + 1;
-        Cx<T>* h0 = bufs + (size_t)(k0 % 3) * HALF;
-        Cx<T>* h1m = bufs + (size_t)(k1h % 3) * HALF - (size_t)HT * PT;     // row t >= HT lives at h1m + t * PT
-        auto trow = [&](int t) { return (t < HT ? h0 : h1m) + t * PT; };
-        const int id = (int)blockIdx.x + i * (int)gridDim.x;
-        const int comp = id / A.tiles_per_comp;
-        const int tidx = id - comp * A.tiles_per_comp;
-        const long long tile_off = (long long)tidx * CX;
-        Cx<T>* base = out + (size_t)comp * A.V + tile_off;
-
-        // ---- z forward, half by half as the halves land ----
-#pragma unroll
-        for (int hh = 0; hh < 2; ++hh) {
-            const int k = 2 * i + hh;
-            mbar_wait(&full[k % 3], (uint32_t)((k / 3) & 1));
-            for (int it = tid; it < CX * HT * SZ::kN2; it += GT) {
-                const int cx = it % CX, t = hh * HT + (it / CX) % HT, n2 = it / (CX * HT);
-                Cx<T>* sp = trow(t) + cx;
-                stage_A_fwd<T, SZ>(n2, twz_f, [&](int p) { return sp[p * PZ]; }, [&](int p, Cx<T> v) { sp[p * PZ] = v; });
-            }
-            __syncthreads();
-            if constexpr (SZ::kN2 > 1) {
-                for (int it = tid; it < CX * HT * SZ::kN1; it += GT) {
-                    const int cx = it % CX, t = hh * HT + (it / CX) % HT, k1 = it / (CX * HT);
-                    Cx<T>* sp = trow(t) + cx;
-                    stage_B<T, SZ, 1, 0>(k1, twz_i, [&](int p) { return sp[p * PZ]; }, [&](int p, Cx<T> v) { sp[p * PZ] = v; }, NoScale());
-                }
-                __syncthreads();
-            }
-        }
-        // ---- t: forward, scale by p2max/(V p2(k)), inverse (lines span both halves) ----
-        {
-            constexpr int NLT = CX * NZ;
-            auto line_momentum = [&](int cx, int zp, T& pxyz, bool& zero_xyz) {
-                const long long sxy = tile_off + cx;
-                const int ypos = int(sxy / A.Lx), xpos = int(sxy - (long long)ypos * A.Lx);
-                const int kx = (xpos / A.x_n2) + A.x_n1 * (xpos % A.x_n2), ky = (ypos / A.y_n2) + A.y_n1 * (ypos % A.y_n2);
-                const int kz = SZ::freq_of_pos(zp);
-                pxyz = reinterpret_cast<const T*>(A.psq_x)[kx] + reinterpret_cast<const T*>(A.psq_y)[ky] +
-                       reinterpret_cast<const T*>(A.psq_z)[kz];
-                zero_xyz = (kx | ky | kz) == 0;
-            };
-            const T* pt = reinterpret_cast<const T*>(A.psq_t);
-            const T num = (T)A.scale_num;
-            static_assert(ST_::kN2 > 1, "the half-tile kernel is meant for two-stage t lines");
-            for (int it = tid; it < NLT * ST_::kN2; it += GT) {
-                const int cx = it % CX, zp = (it / CX) % NZ, n2 = it / NLT;
-                const int off = cx + zp * PZ;
-                stage_A_fwd<T, ST_>(n2, twt_f, [&](int p) { return trow(p)[off]; }, [&](int p, Cx<T> v) { trow(p)[off] = v; });
-            }
-            __syncthreads();
-            for (int it = tid; it < NLT * ST_::kN1; it += GT) {
-                const int cx = it % CX, zp = (it / CX) % NZ, k1 = it / NLT;
-                const int off = cx + zp * PZ;
-                T pxyz; bool zero_xyz;
-                line_momentum(cx, zp, pxyz, zero_xyz);
-                auto scale = [&](int k2) -> T {
-                    const int kt = k1 + ST_::kN1 * k2;
-                    const T den = pxyz + __ldg(pt + kt);
-                    return (zero_xyz && kt == 0) ? T(0) : fast_div(num, den);
-                };
-                stage_B<T, ST_, 1, 1>(k1, twt_i, [&](int p) { return trow(p)[off]; }, [&](int p, Cx<T> v) { trow(p)[off] = v; }, scale);
-            }
-            __syncthreads();
-            for (int it = tid; it < NLT * ST_::kN2; it += GT) {
-                const int cx = it % CX, zp = (it / CX) % NZ, n2 = it / NLT;
-                const int off = cx + zp * PZ;
-                stage_A_inv<T, ST_>(n2, [&](int p) { return trow(p)[off]; }, [&](int p, Cx<T> v) { trow(p)[off] = v; });
-            }
-            __syncthreads();
-        }
-        // ---- z inverse: B' in shared memory, A' straight to global (natural layout) ----
-        if constexpr (SZ::kN2 > 1) {
-            for (int it = tid; it < CX * NT * SZ::kN1; it += GT) {
-                const int cx = it % CX, t = (it / CX) % NT, k1 = it / (CX * NT);
-                Cx<T>* sp = trow(t) + cx;
-                stage_B<T, SZ, 0, 1>(k1, twz_i, [&](int p) { return sp[p * PZ]; }, [&](int p, Cx<T> v) { sp[p * PZ] = v; }, NoScale());
-            }
-            __syncthreads();
-        }
-        for (int it = tid; it < CX * NT * SZ::kN2; it += GT) {
-            const int cx = it % CX, t = (it / CX) % NT, n2 = it / (CX * NT);
-            Cx<T>* gp = base + cx + (size_t)t * gt;
-            const Cx<T>* sp = trow(t) + cx;
-            stage_A_inv<T, SZ>(n2, [&](int p) { return sp[p * PZ]; }, [&](int p, Cx<T> v) { st_cx(gp + (size_t)p * gz, v); });
-        }
-        // ---- both half buffers go back to the TMA unit: halves 2i+3 (next tile's second) and 2i+4 ----
-        fence_proxy_async();
-        __syncthreads();
-        if (tid == 0) {
-            if (2 * i + 3 < 2 * my_tiles) issue(2 * i + 3);
-            if (2 * i + 4 < 2 * my_tiles) issue(2 * i + 4);
-        }
     }
 }
 

@@ -19,7 +19,7 @@
 // uniform across a warp, so the factors are literals selected by a warp-uniform switch (mul_tw<>, no table loads:
 // the load/store unit is left to the shared-memory traffic).  When the t line fits the B x C block (D = 1: 48 x 8,
 // 48 x 4, 48 x 6) P2, P3 and P4 are ONE pass.  The spectrum order is that of lgf_fft_ct.cuh (position k1*N2 + k2 holds
-// frequency k1 + N1*k2); tiles, layout B, ring and half-tile ring are those of lgf_fft_pipe.cuh.
+// frequency k1 + N1*k2); tiles, layout B and the ring are those of lgf_fft_pipe.cuh.
 // Product code (sm_100a); shares nothing with oracle/.
 #pragma once
 #include <cuda.h>
@@ -296,91 +296,8 @@ fft_zt_pipe3(const Cx<T>* inB, Cx<T>* out, const __grid_constant__ ZtArgs A, con
     }
 }
 
-// Half-tile ring (the structure of fft_zt_pipe_halves) for planes too large for a ring of whole tiles: 64 x 64 with
-// CX = 2 in fp64 / CX = 4 in fp32 is 133 KB.  The tile travels as two t-halves through three half-tile buffers; P1 runs
-// on each half as it lands (z lines live inside one t row).
-template <typename T, class SZ, class ST_, int CX, int GT>
-__global__ void __launch_bounds__(GT, 1)
-fft_zt_pipe3_halves(const Cx<T>* inB, Cx<T>* out, const __grid_constant__ ZtArgs A, const int* done) {
-    pdl_entry();
-    extern __shared__ __align__(128) unsigned char pipe_smem[];
-    if (done && *reinterpret_cast<const volatile int*>(done)) return;
-    typedef Zt3<T, SZ, ST_, CX> P;
-    constexpr int NZ = SZ::kN, NT = ST_::kN, PT = CX * (NZ + 1), HT = NT / 2, HALF = PT * HT;
-    static_assert(NT % 2 == 0 && (HALF * sizeof(Cx<T>)) % 16 == 0 && GT % 32 == 0, "half tiles");
-    static_assert(P::D > 1, "the half-tile kernel is meant for two-stage t lines");
-    Cx<T>* bufs = reinterpret_cast<Cx<T>*>(pipe_smem);
-    uint64_t* full = reinterpret_cast<uint64_t*>(pipe_smem + sizeof(Cx<T>) * (size_t)3 * HALF);
-    const int tid = threadIdx.x;
-    const int ntiles = 4 * A.tiles_per_comp;
-    const int my_tiles = (int)blockIdx.x < ntiles ? (ntiles - (int)blockIdx.x + (int)gridDim.x - 1) / (int)gridDim.x : 0;
-    const long long gz = A.LxLy, gt = A.LxLy * NZ;
-
-    auto issue = [&](int k) {             // half k = 2 * (tile index of this CTA) + (0 | 1)
-        const int buf = k % 3;
-        const size_t id = (size_t)blockIdx.x + (size_t)(k >> 1) * gridDim.x;
-        const uint32_t bytes = (uint32_t)(HALF * sizeof(Cx<T>));
-        mbar_arrive_expect_tx(&full[buf], bytes);
-        bulk_g2s(bufs + (size_t)buf * HALF, inB + id * (size_t)(2 * HALF) + (size_t)(k & 1) * HALF, bytes, &full[buf]);
-    };
-    if (tid == 0) {
-        for (int b = 0; b < 3; ++b) mbar_init(&full[b], 1);
-        mbar_fence_init();
-        for (int k = 0; k < 3 && k < 2 * my_tiles; ++k) issue(k);
-    }
-    __syncthreads();
-
-    for (int i = 0; i < my_tiles; ++i) {
-        Cx<T>* h0 = bufs + (size_t)((2 * i) % 3) * HALF;
-        // row t >= HT lives at h0 + t * PT + hoff (hoff = distance of the second half's buffer from where it would sit
-        // behind the first)
-        const int hoff = (int)((bufs + (size_t)((2 * i + 1) % 3) * HALF - (size_t)HT * PT) - h0);
-        auto row = [&](int t) { return h0 + t * PT + (t >= HT ? hoff : 0); };
-        const int id = (int)blockIdx.x + i * (int)gridDim.x;
-        const int comp = id / A.tiles_per_comp;
-        const int tidx = id - comp * A.tiles_per_comp;
-        const long long tile_off = (long long)tidx * CX;
-        Cx<T>* base = out + (size_t)comp * A.V + tile_off;
-
-        {
-            constexpr int IH = CX * HT * P::B;           // P1 items of one half
-            const int k0 = 2 * i, k1 = 2 * i + 1;
-            if constexpr (GT >= 2 * IH) {
-                // enough threads for both halves at once: the upper half of the CTA takes the second half-tile
-                const int hh = tid >= GT / 2 ? 1 : 0;
-                const int k = hh ? k1 : k0;
-                mbar_wait(&full[k % 3], (uint32_t)((k / 3) & 1));
-                for (int it = tid - hh * (GT / 2); it < IH; it += GT / 2) P::template p1<HT>(it, hh * HT, row);
-                const int ko = hh ? k0 : k1;             // every thread observes both barriers before the later passes
-                mbar_wait(&full[ko % 3], (uint32_t)((ko / 3) & 1));
-            } else {
-                mbar_wait(&full[k0 % 3], (uint32_t)((k0 / 3) & 1));
-                for (int it = tid; it < IH; it += GT) P::template p1<HT>(it, 0, row);
-                mbar_wait(&full[k1 % 3], (uint32_t)((k1 / 3) & 1));
-                for (int it = tid; it < IH; it += GT) P::template p1<HT>(it, HT, row);
-            }
-        }
-        __syncthreads();
-        auto row2 = [&](int lo, int hi) { return row(lo + P::D * hi); };
-        for (int it = tid; it < P::kItems2; it += GT) P::template p2<false, P::D>(it, row2);
-        __syncthreads();
-        for (int it = tid; it < P::kItems3; it += GT) P::template p3<false>(it, row2, A, tile_off);
-        __syncthreads();
-        for (int it = tid; it < P::kItems2; it += GT) P::template p4<false, P::D>(it, row2);
-        __syncthreads();
-        for (int it = tid; it < P::kItems1; it += GT) P::p5(it, row, base, gz, gt);
-        // ---- both half buffers go back to the TMA unit: halves 2i+3 (next tile's second) and 2i+4 ----
-        fence_proxy_async();
-        __syncthreads();
-        if (tid == 0) {
-            if (2 * i + 3 < 2 * my_tiles) issue(2 * i + 3);
-            if (2 * i + 4 < 2 * my_tiles) issue(2 * i + 4);
-        }
-    }
-}
-
 // Quarter-tile ring with asynchronous output for planes too large for a ring of whole tiles (64 x 64: a CX = 2 fp64 /
-// CX = 4 fp32 tile is 133 KB).  ncu on fft_zt_pipe3_halves at 64^4 (profiles/r2_k3_*): 43 % of the kernel's warp-time
+// CX = 4 fp32 tile is 133 KB).  ncu on a half-tile ring with per-thread stores at 64^4 (profiles/r2_k3_*): 43 % of the kernel's warp-time
 // sat in P5's scattered 32-byte global stores and the barrier behind them (stall_lg: every STG.128 of a warp is 16 tag
 // requests), and the second half-tile's fetch was exposed behind every tile.  Here
 //  * P5 runs in place in shared memory and the TMA unit stores the tile (cp.async.bulk.tensor, SASS UTMASTG: a 5-D box

@@ -15,7 +15,8 @@ const XyPipeEntry* xy_pipe_table_f32(int* n) {
         XyP<T, 32, 32, 32, 32, 8, 256, 2, 3>::entry(),
         XyP<T, 48, 8, 48, 8, 2, 192, 2, 4>::entry(),
         XyP<T, 48, 8, 48, 8, 1, 256, 2, 4>::entry(),
-        XyP<T, 64, 8, 64, 8, 1, 256, 2, 4>::entry(),
+        XyPIO<T, 64, 8, 64, 8, 1, 256, 2, 4>::entry(),      // K2: 32-byte chunks of layout B leave through the TMA unit
+        XyP<T, 64, 8, 64, 8, 1, 256, 2, 4>::entry(),        // K4 (and K2 as variant 1)
     };
     *n = (int)(sizeof(tab) / sizeof(tab[0]));
     return tab;
@@ -27,21 +28,14 @@ const ZtPipeEntry* zt_pipe_table_f32(int* n) {
         ZtP<T, 32, 32, 32, 32, 4, 128, 4, 6>::entry(),
         ZtP<T, 32, 32, 32, 32, 4, 128, 2, 4>::entry(),
         ZtP<T, 32, 32, 32, 32, 8, 256, 2, 3>::entry(),
-        ZtP3<T, 48, 16, 8, 8, 8, 192, 2, 4>::entry(),          // three register stages (lgf_fft_pipe3.cuh): 3 passes instead of 5
+        ZtP3<T, 48, 16, 8, 8, 8, 192, 2, 4>::entry(),
         ZtP3<T, 48, 16, 8, 8, 8, 128, 3, 4>::entry(),
         ZtP<T, 48, 8, 8, 8, 8, 128, 3, 4>::entry(),
         // the paper's other finite-temperature shapes 48^3 x N_t, N_t = 4, 6, 12
         ZtP3<T, 48, 16, 4, 4, 8, 192, 2, 4>::entry(),
-        ZtP<T, 48, 8, 4, 4, 8, 128, 3, 4>::entry(),
         ZtP3<T, 48, 16, 6, 6, 8, 192, 2, 4>::entry(),
-        ZtP<T, 48, 8, 6, 6, 8, 128, 3, 4>::entry(),
         ZtP<T, 48, 8, 12, 12, 8, 128, 2, 3>::entry(),
-        ZtP<T, 48, 8, 8, 8, 8, 256, 2, 4>::entry(),
-        ZtP3Q<T, 64, 16, 64, 4, 4, 512>::entry(),             // quarter ring, TMA tensor store of the output
-        ZtP3H<T, 64, 16, 64, 4, 4, 512>::entry(),             // 5 shared-memory passes instead of 7
-        ZtP3<T, 64, 16, 64, 4, 4, 512, 1, 1>::entry(),
-        ZtPH<T, 64, 8, 64, 8, 4, 512>::entry(),
-        ZtP<T, 64, 8, 64, 8, 4, 512, 1, 1>::entry(),
+        ZtP3Q<T, 64, 16, 64, 4, 4, 512>::entry(),
     };
     *n = (int)(sizeof(tab) / sizeof(tab[0]));
     return tab;

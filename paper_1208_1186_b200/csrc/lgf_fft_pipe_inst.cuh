@@ -12,11 +12,12 @@ struct XyPipeEntry {
     int nx, ny;
     int x_n1, y_n1;          // first-stage radices (digit-swapped spectrum order, see lgf_fft_ct.cuh)
     int pb;                  // planes per tile
-    int threads;             // GT * NG
+    int threads;             // GT * NG (+ 32 for the kernels with an I/O warp)
     int nbuf;
     size_t smem;
     const void* k_fwd;       // fft_xy_pipe<..., -1, ...>  natural -> layout B
-    const void* k_inv;       // fft_xy_pipe<..., +1, ...>  natural -> natural
+    const void* k_inv;       // fft_xy_pipe<..., +1, ...>  natural -> natural (nullptr: forward-only entry)
+    int io;                  // 1: fft_xy_pipe_io (I/O warp, TMA tensor stores into layout B; takes the layout-B CUtensorMap)
 };
 struct ZtPipeEntry {
     int nz, nt;
@@ -25,8 +26,9 @@ struct ZtPipeEntry {
     int nbuf;
     size_t smem;
     const void* kernel;      // fft_zt_pipe<...>  layout B -> natural
-    // quarter-ring kernel (fft_zt_pipe3q): layout B holds the t rows quarter by quarter (XyPipeArgs::perm_*; perm_c x perm_d = its split of the t lines),
-    // and the kernel takes a fifth argument, the CUtensorMap of its output (tstore = 1); 0, 1, nt otherwise
+    // tstore = 1: the quarter-ring kernel fft_zt_pipe3q, which stores quarter tiles through the TMA unit and takes the 5-D
+    // CUtensorMap of the natural-layout Delta~ field as its fifth argument; layout B then holds the t rows quarter by
+    // quarter (XyPipeArgs::perm_*; perm_c x perm_d = the kernel's split of the t lines).  0, 1, nt for the ring kernels.
     int tstore, perm_c, perm_d;
 };
 

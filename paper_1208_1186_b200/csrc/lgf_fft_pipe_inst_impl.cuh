@@ -2,6 +2,7 @@
 #pragma once
 #include "lgf_fft_pipe.cuh"
 #include "lgf_fft_pipe3.cuh"
+#include "lgf_fft_pipe_io.cuh"
 #include "lgf_fft_pipe_inst.cuh"
 
 namespace lgf {
@@ -16,7 +17,20 @@ struct XyP {
     static XyPipeEntry entry() {
         return XyPipeEntry{NX, NY, X1, Y1, PB, GT * NG, NBUF, kSmem,
                            (const void*)&fft_xy_pipe<T, SX, SY, -1, PB, GT, NG, NBUF>,
-                           (const void*)&fft_xy_pipe<T, SX, SY, +1, PB, GT, NG, NBUF>};
+                           (const void*)&fft_xy_pipe<T, SX, SY, +1, PB, GT, NG, NBUF>, 0};
+    }
+};
+
+// K2 through the I/O warp and TMA tensor stores (fft_xy_pipe_io); K4 of such a lattice runs on a plain XyP entry
+template <typename T, int NX, int X1, int NY, int Y1, int PB, int GT, int NG, int NBUF>
+struct XyPIO {
+    typedef LineSplit<NX, X1> SX;
+    typedef LineSplit<NY, Y1> SY;
+    static constexpr size_t kSmem = sizeof(Cx<T>) * (size_t)NBUF * PB * NX * NY + 16 * NBUF;
+    static_assert(kSmem <= 227 * 1024, "tile ring exceeds shared memory");
+    static XyPipeEntry entry() {
+        return XyPipeEntry{NX, NY, X1, Y1, PB, GT * NG + 32, NBUF, kSmem,
+                           (const void*)&fft_xy_pipe_io<T, SX, SY, -1, PB, GT, NG, NBUF>, nullptr, 1};
     }
 };
 
@@ -32,19 +46,6 @@ struct ZtP {
     }
 };
 
-// half-tile ring variant of K3 (fft_zt_pipe_halves): three half-tile buffers
-template <typename T, int NZ, int Z1, int NT, int T1, int CX, int GT>
-struct ZtPH {
-    typedef LineSplit<NZ, Z1> SZ;
-    typedef LineSplit<NT, T1> ST_;
-    static constexpr size_t kSmem = sizeof(Cx<T>) * (size_t)3 * CX * (NZ + 1) * (NT / 2) + 8 * 3;
-    static_assert(kSmem <= 227 * 1024, "half-tile ring exceeds shared memory");
-    static_assert((CX & (CX - 1)) == 0, "CX must be a power of two");
-    static ZtPipeEntry entry() {
-        return ZtPipeEntry{NZ, NT, CX, GT, 3, kSmem, (const void*)&fft_zt_pipe_halves<T, SZ, ST_, CX, GT>, 0, 1, NT};
-    }
-};
-
 // three-register-stage K3 (lgf_fft_pipe3.cuh): ring of whole tiles / half-tile ring
 template <typename T, int NZ, int Z1, int NT, int T1, int CX, int GT, int NG, int NBUF>
 struct ZtP3 {
@@ -57,18 +58,6 @@ struct ZtP3 {
         return ZtPipeEntry{NZ, NT, CX, GT * NG, NBUF, kSmem, (const void*)&fft_zt_pipe3<T, SZ, ST_, CX, GT, NG, NBUF>, 0, 1, NT};
     }
 };
-template <typename T, int NZ, int Z1, int NT, int T1, int CX, int GT>
-struct ZtP3H {
-    typedef LineSplit<NZ, Z1> SZ;
-    typedef LineSplit<NT, T1> ST_;
-    static constexpr size_t kSmem = sizeof(Cx<T>) * (size_t)3 * CX * (NZ + 1) * (NT / 2) + 8 * 3;
-    static_assert(kSmem <= 227 * 1024, "half-tile ring exceeds shared memory");
-    static_assert((CX & (CX - 1)) == 0, "CX must be a power of two");
-    static ZtPipeEntry entry() {
-        return ZtPipeEntry{NZ, NT, CX, GT, 3, kSmem, (const void*)&fft_zt_pipe3_halves<T, SZ, ST_, CX, GT>, 0, 1, NT};
-    }
-};
-
 // quarter ring + TMA tensor store (fft_zt_pipe3q)
 template <typename T, int NZ, int Z1, int NT, int T1, int CX, int GT>
 struct ZtP3Q {
