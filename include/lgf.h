@@ -51,8 +51,10 @@ enum {
     LGF_EINVAL = -1,       /* null pointer, L_mu < 2, bad enum, alpha <= 0, n < 0, workspace too small/misaligned */
     LGF_EUNSUPPORTED = -2, /* an L_mu with a prime factor other than 2 or 3, or a transform tile that
                               does not fit in shared memory (see lgf_workspace_bytes)               */
-    LGF_ESTATE = -3,       /* iterate / fix / measure / store before load                          */
-    LGF_ECUDA = -4         /* a CUDA call failed (no device, launch error, ...); see lgf_last_error */
+    LGF_ESTATE = -3,       /* iterate / fix / measure / store before load; any call but lgf_wait while an
+                              lgf_iterate_async is pending */
+    LGF_ECUDA = -4,        /* a CUDA call failed (no device, launch error, ...); see lgf_last_error */
+    LGF_ENOMEM = -5        /* a host allocation failed */
 };
 
 /* Result of a measurement or of a run.  theta and F are those of the links held by the context when
@@ -64,11 +66,11 @@ typedef struct {
     int32_t converged;  /* theta < theta_tol (lgf_fix only; 0 otherwise) */
 } lgf_result;
 
-/* Bytes of device workspace lgf_create needs for this lattice: two link buffers in the device
- * layout (the fused update kernel writes out of place; the default path uses only the first), three
- * packed Delta-sized fields (4 complex per site: Delta, the layout-B spectrum between
- * K2 and K3, Delta~), reduction partials, twiddle and p^2 tables, boundary staging.  About
- * (8 n_l + 24 (1 + 1/(3 Lz))) w bytes per site.  Returns 0 if the arguments are invalid or unsupported. */
+/* Bytes of device workspace lgf_create needs for this lattice: the links in the device layout, two packed
+ * Delta-sized fields (4 complex per site: Delta / Delta~ and the layout-B spectrum between
+ * K2 and K3), reduction partials, twiddle and p^2 tables, boundary staging.  About
+ * (4 n_l + 16 (1 + 1/(2 Lz))) w bytes per site.  Returns 0 exactly when lgf_create would refuse the lattice:
+ * invalid arguments, an extent that is not 2^a 3^b, V >= 2^31, or a transform tile that does not fit on chip. */
 size_t lgf_workspace_bytes(const int32_t L[4], int precision, int storage);
 
 /* Create a context.  `workspace_dev` is DEVICE memory of at least lgf_workspace_bytes(...) bytes,

@@ -44,6 +44,8 @@ def lib() -> ctypes.CDLL:
         _lib.orc_iterate.argtypes = [_ip, _dp, ctypes.c_int64, ctypes.c_double, _dp, _dp]
         _lib.orc_build_g.argtypes = [_ip, _dp, ctypes.c_double, _dp]
         _lib.orc_two_row_roundtrip.argtypes = [ctypes.c_int64, _dp, _dp]
+        _lib.orc_wilson_lines.argtypes = [_ip, _dp, _dp]
+        _lib.orc_singlet_correlator.argtypes = [_ip, _dp, _dp]
     return _lib
 
 
@@ -176,3 +178,21 @@ def fix(L, U, alpha: float, theta_tol: float, max_iter: int):
                       ctypes.byref(t), ctypes.byref(F), _d(th), _d(Fh))
     return (U.view(np.complex128).reshape(_vol(L), 4, 3, 3), int(n), t.value, F.value,
             th[:n + 1].copy(), Fh[:n + 1].copy())
+
+
+def wilson_lines(L, U) -> np.ndarray:
+    """Temporal Wilson lines W(x) = prod_t U_t(x, t) -> complex [Vs, 3, 3], Vs = Lx Ly Lz."""
+    U = _f64(U)
+    Vs = _vol(L) // int(L[3])
+    out = np.empty(Vs * 18, dtype=np.float64)
+    lib().orc_wilson_lines(_L(L), _d(U), _d(out))
+    return out.view(np.complex128).reshape(Vs, 3, 3)
+
+
+def singlet_correlator(L, U) -> np.ndarray:
+    """C(r) = (1/(3 Vs)) sum_x Tr[W(x + r) W(x)^+] -> complex [Vs] (x fastest), by the direct double sum (eq. (1))."""
+    U = _f64(U)
+    Vs = _vol(L) // int(L[3])
+    out = np.empty(Vs * 2, dtype=np.float64)
+    lib().orc_singlet_correlator(_L(L), _d(U), _d(out))
+    return out.view(np.complex128)

@@ -19,6 +19,11 @@
 // E[theta] = 128/9 on Haar links; position-space convolution brute force.
 // "parity unpinned": the final links of a rough configuration have no external truth; they
 // are validated only through the pins above.
+// The step after the path (eq. (1)): temporal Wilson lines and the singlet
+// correlator of ONE configuration, written out as the definition (ordered product along t; direct double sum over
+// the spatial lattice).  Pins (tests/test_oracle_correlator.py): W = 1 and C = 1 on the unit field; C(0) = 1;
+// C(-r) = conj C(r); sum_r C(r) = |sum_x W(x)|_F^2 / (3 Vs); Tr W against a torch restatement of the Polyakov loop;
+// covariance W -> g(x,0) W g(x,0)^+ under a gauge transform, invariance of C under x-independent transforms.
 //
 // Loops carry `#pragma omp parallel for` over sites / FFT lines only; every reduction is a
 // serial compensated sum over a per-site array, so results are bit-identical for any thread
@@ -319,6 +324,45 @@ void update_links(const Lat& lat, const double* U, const double* g, double* Unew
     }
 }
 
+// Temporal Wilson line ("W(.) is the temporal Wilson line"): W(x) = U_t(x,0) U_t(x,1) ... U_t(x,Lt-1),
+// the ordered product of the t-links at spatial site x = (x,y,z); xs = x + Lx (y + Ly z).
+void wilson_lines(const Lat& lat, const double* U, double* W) {
+    const int64_t Vs = lat.V / lat.L[3];
+#pragma omp parallel for schedule(static)
+    for (int64_t xs = 0; xs < Vs; ++xs) {
+        Mat3 w = load(U + ((xs + 0 * Vs) * 4 + 3) * 18);
+        for (int t = 1; t < lat.L[3]; ++t) w = mul(w, load(U + ((xs + (int64_t)t * Vs) * 4 + 3) * 18));
+        store(W + xs * 18, w);
+    }
+}
+
+// Singlet correlator of one configuration, eq. (1) of PAPER.md:33 with the ensemble average replaced by the average
+// over the spatial lattice:  C(r) = (1/(3 Vs)) sum_x Tr[ W(x + r) W(x)^+ ],  r on the periodic spatial lattice.
+// Direct O(Vs^2) double sum, compensated per r.
+void singlet_correlator(const Lat& lat, const double* U, double* C) {
+    const int64_t Vs = lat.V / lat.L[3];
+    std::vector<double> W((size_t)Vs * 18);
+    wilson_lines(lat, U, W.data());
+    const int Lx = lat.L[0], Ly = lat.L[1], Lz = lat.L[2];
+#pragma omp parallel for schedule(static)
+    for (int64_t r = 0; r < Vs; ++r) {
+        const int rx = int(r % Lx), ry = int((r / Lx) % Ly), rz = int(r / ((int64_t)Lx * Ly));
+        std::vector<double> re((size_t)Vs), im((size_t)Vs);
+        for (int64_t xs = 0; xs < Vs; ++xs) {
+            const int x = int(xs % Lx), y = int((xs / Lx) % Ly), z = int(xs / ((int64_t)Lx * Ly));
+            const int64_t xr = (x + rx) % Lx + (int64_t)Lx * ((y + ry) % Ly + (int64_t)Ly * ((z + rz) % Lz));
+            const Mat3 a = load(W.data() + xr * 18), b = load(W.data() + xs * 18);
+            cplx tr = 0;                       // Tr[a b^+] = sum_ij a_ij conj(b_ij)
+            for (int i = 0; i < 3; ++i)
+                for (int j = 0; j < 3; ++j) tr += a.a[i][j] * std::conj(b.a[i][j]);
+            re[xs] = tr.real();
+            im[xs] = tr.imag();
+        }
+        C[2 * r] = compensated_sum(re) / (3.0 * (double)Vs);
+        C[2 * r + 1] = compensated_sum(im) / (3.0 * (double)Vs);
+    }
+}
+
 }  // namespace
 
 extern "C" {
@@ -428,5 +472,9 @@ int64_t orc_fix(const int32_t* L, double* U, double alpha, double theta_tol, int
     *F_out = F;
     return n;
 }
+
+
+void orc_wilson_lines(const int32_t* L, const double* U, double* W) { wilson_lines(Lat(L), U, W); }
+void orc_singlet_correlator(const int32_t* L, const double* U, double* C) { singlet_correlator(Lat(L), U, C); }
 
 }  // extern "C"

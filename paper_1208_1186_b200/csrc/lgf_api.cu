@@ -38,6 +38,14 @@ int cuda_fail(cudaError_t e, const char* what) {
         if (e__ != cudaSuccess) return cuda_fail(e__, #call); \
     } while (0)
 
+// Developer A/B knobs (LGF_ZBLOCK, LGF_SITE_TILE, LGF_FUSED, ...; DESIGN.md §6 "A/B knobs") are read only when
+// LGF_DEVKNOBS=1 is set: a production process cannot change which kernels run through a stray environment variable.
+const char* knob(const char* name) {
+    static const bool enabled = [] { const char* e = getenv("LGF_DEVKNOBS"); return e && atoi(e) != 0; }();
+    return enabled ? getenv(name) : nullptr;
+}
+bool fused_requested() { const char* e = knob("LGF_FUSED"); return e && atoi(e) != 0; }
+
 constexpr size_t kAlign = 256;
 size_t align_up(size_t v) { return (v + kAlign - 1) / kAlign * kAlign; }
 
@@ -94,12 +102,15 @@ bool valid_args(const int32_t L[4], int precision, int storage) {
     if (!L) return false;
     if (precision != LGF_F32 && precision != LGF_F64) return false;
     if (storage != LGF_REAL18 && storage != LGF_REAL12) return false;
-    for (int i = 0; i < 4; ++i)
+    long long V = 1;
+    for (int i = 0; i < 4; ++i) {
         if (L[i] < 2 || L[i] > 4096) return false;
-    return true;
+        V *= L[i];
+    }
+    return V < (1ll << 31);      // the site kernels index sites with 32-bit integers
 }
 
-Layout make_layout(const int32_t L[4], int precision, int storage) {
+Layout make_layout(const int32_t L[4], int precision, int storage, bool fused) {
     Layout lo;
     const size_t w = precision == LGF_F64 ? 8 : 4;
     const size_t V = (size_t)L[0] * L[1] * L[2] * L[3];
@@ -124,13 +135,13 @@ Layout make_layout(const int32_t L[4], int precision, int storage) {
     for (int i = 0; i < 4; ++i) { lo.tw[i] = off; off += align_up((size_t)L[i] * 2 * w); }
     for (int i = 0; i < 4; ++i) { lo.twi[i] = off; off += align_up((size_t)L[i] * 2 * w); }
     for (int i = 0; i < 4; ++i) { lo.psq[i] = off; off += align_up((size_t)L[i] * w); }
-    // two link buffers: the fused update kernel writes the new field out of place (DevState::cur)
+    // the fused update kernel (opt-in) writes the new field out of place into a second link buffer (DevState::cur)
     lo.links_bytes = align_up(4 * (size_t)(storage / 2) * V * 2 * w);
-    lo.links = off; off += 2 * lo.links_bytes;
+    lo.links = off; off += (fused ? 2 : 1) * lo.links_bytes;
     lo.delta = off; off += align_up(4 * V * 2 * w);
     // layout-B spectrum between K2 and K3 (pipelined FFT path): tiles padded by one z entry per t row
     lo.delta2 = off; off += align_up(4 * (V / L[2]) * (size_t)(L[2] + 1) * 2 * w);
-    lo.delta3 = off; off += align_up(4 * V * 2 * w);   // Delta of the new links (fused path: K1/K51 out, K2 in)
+    lo.delta3 = off; off += fused ? align_up(4 * V * 2 * w) : 0;   // Delta of the new links (fused path: K1/K51 out, K2 in)
     const size_t stage_sites = V < (size_t)kStageSites ? V : (size_t)kStageSites;
     lo.staging = off; off += align_up(stage_sites * 36 * 2 * w);
     lo.total = off;
@@ -245,7 +256,7 @@ void set_walk(Geom& g, int tz, size_t link_bytes_per_site, size_t slice_limit = 
         zb = (int)(((size_t)16 << 20) / per_ztile);
         if (zb < 1) zb = 1;
     }
-    const char* e = getenv("LGF_ZBLOCK");
+    const char* e = knob("LGF_ZBLOCK");
     if (e) zb = atoi(e) > 0 ? atoi(e) : g.nb[2];
     if (zb > g.nb[2]) zb = g.nb[2];
     while (g.nb[2] % zb) --zb;
@@ -343,10 +354,10 @@ bool plan_passes(lgf_ctx* c) {
     if (!c->xy_pipe) c->zt_pipe = nullptr;
     c->xy_pipe_inv = c->xy_pipe ? find_xy_pipe_inv(c->precision, L[0], L[1], c->xy_pipe) : nullptr;
     {   // LGF_FFT_PIPE=0: fall back to the one-tile-per-CTA kernels (A/B knob)
-        const char* e = getenv("LGF_FFT_PIPE");
+        const char* e = knob("LGF_FFT_PIPE");
         if (e && atoi(e) == 0) c->xy_pipe = nullptr, c->zt_pipe = nullptr;
     }
-    if (getenv("LGF_FORCE_GENERIC_FFT")) c->xy_ct = nullptr, c->zt_ct = nullptr, c->xy_pipe = nullptr, c->zt_pipe = nullptr;
+    if (knob("LGF_FORCE_GENERIC_FFT")) c->xy_ct = nullptr, c->zt_ct = nullptr, c->xy_pipe = nullptr, c->zt_pipe = nullptr;
     if (c->xy_ct) {
         c->xy_args.twx_fwd = c->axis[0].tw_fwd; c->xy_args.twx_inv = c->axis[0].tw_inv;
         c->xy_args.twy_fwd = c->axis[1].tw_fwd; c->xy_args.twy_inv = c->axis[1].tw_inv;
@@ -390,6 +401,21 @@ bool plan_passes(lgf_ctx* c) {
         A.y_n2 = L[1] / A.y_n1;
     }
     return true;
+}
+
+// The host-only part of lgf_create's planning, so that lgf_workspace_bytes and lgf_create agree on what is supported:
+// does every transform tile of this lattice fit in shared memory / the thread limit?
+bool tiles_fit(const int32_t L[4], int precision) {
+    lgf_ctx* t = new (std::nothrow) lgf_ctx();
+    if (!t) return false;
+    memset(static_cast<void*>(t), 0, sizeof(*t));
+    for (int i = 0; i < 4; ++i) t->L[i] = L[i];
+    t->precision = precision;
+    t->V = (long long)L[0] * L[1] * L[2] * L[3];
+    t->wbytes = precision == LGF_F64 ? 8 : 4;
+    const bool ok = plan_passes(t);
+    delete t;
+    return ok;
 }
 
 typedef CUresult (*TensorMapEncodeFn)(CUtensorMap*, CUtensorMapDataType, cuuint32_t, void*, const cuuint64_t*, const cuuint64_t*,
@@ -542,9 +568,8 @@ struct Impl {
     static int plan_fused(lgf_ctx* c) {
         c->fused_tile = -1;
         if (!c->xy_pipe) return LGF_OK;                    // the fused path rides on the pipelined FFT buffers
-        const char* e = getenv("LGF_FUSED");
-        if (!e || atoi(e) == 0) return LGF_OK;             // opt-in (LGF_FUSED=1) until it beats K5 + K1 everywhere
-        const char* ft = getenv("LGF_FUSED_TILE");
+        if (!fused_requested()) return LGF_OK;             // opt-in (LGF_DEVKNOBS=1 LGF_FUSED=1) until it beats K5 + K1 everywhere
+        const char* ft = knob("LGF_FUSED_TILE");
         const FusedEntry* tab = fused_entries();
         for (int i = 0; i < kNumFused; ++i) {
             if (ft && atoi(ft) != i) continue;
@@ -862,8 +887,9 @@ const char* lgf_strerror(int code) {
         case LGF_OK: return "ok";
         case LGF_EINVAL: return "invalid argument";
         case LGF_EUNSUPPORTED: return "unsupported lattice (extent not 2^a 3^b, or transform tile exceeds shared memory)";
-        case LGF_ESTATE: return "no links loaded";
+        case LGF_ESTATE: return "no links loaded, or lgf_iterate_async pending (call lgf_wait first)";
         case LGF_ECUDA: return "CUDA error (see lgf_last_error)";
+        case LGF_ENOMEM: return "host allocation failed";
         default: return "unknown error";
     }
 }
@@ -873,14 +899,15 @@ size_t lgf_workspace_bytes(const int32_t L[4], int precision, int storage) {
     Axis ax;
     for (int i = 0; i < 4; ++i)
         if (!factor23(L[i], &ax)) return 0;
-    return make_layout(L, precision, storage).total;
+    if (!tiles_fit(L, precision)) return 0;
+    return make_layout(L, precision, storage, fused_requested()).total;
 }
 
 static int create_common(const int32_t L[4], int precision, int storage, void* ws, size_t ws_bytes, bool owns,
                          void* stream, lgf_ctx** out) {
     lgf_ctx* c = new (std::nothrow) lgf_ctx();
-    if (!c) return LGF_EINVAL;
-    memset(c, 0, sizeof(*c));
+    if (!c) return LGF_ENOMEM;
+    memset(static_cast<void*>(c), 0, sizeof(*c));
     for (int i = 0; i < 4; ++i) c->L[i] = L[i];
     c->precision = precision;
     c->storage = storage;
@@ -889,19 +916,19 @@ static int create_common(const int32_t L[4], int precision, int storage, void* w
     c->ws = reinterpret_cast<char*>(ws);
     c->owns_ws = owns;
     c->stream = reinterpret_cast<cudaStream_t>(stream);
-    c->lo = make_layout(L, precision, storage);
+    c->lo = make_layout(L, precision, storage, fused_requested());
     c->pending_n = -1;
     {
-        const char* e = getenv("LGF_PDL");
+        const char* e = knob("LGF_PDL");
         // measured: 8^4 22.6 -> 20.5 us per iteration, 16^4 32.8 -> 32.0 us, but 32^4 fp64-12 315 -> 381 us
         // with every edge programmatic (no single edge gains more than 1.5 us there), so: launch-bound lattices only
         c->pdl_enabled = e ? atoi(e) != 0 : c->V <= 65536;
-        e = getenv("LGF_PDL_MASK");
+        e = knob("LGF_PDL_MASK");
         c->pdl_mask = e ? atoi(e) : 0x3e;
     }
     {   // thread-per-site tiling: widest x tile that divides Lx (LGF_SITE_TILE overrides, A/B knob)
         int t = (L[0] % 32 == 0) ? 4 : ((L[0] % 16 == 0) ? 1 : 0);
-        const char* e = getenv("LGF_SITE_TILE");
+        const char* e = knob("LGF_SITE_TILE");
         if (e && atoi(e) >= 0 && atoi(e) < kNumSiteTiles) t = atoi(e);
         c->site_tile = t;
         int n = 1;
@@ -914,13 +941,13 @@ static int create_common(const int32_t L[4], int precision, int storage, void* w
     set_walk(c->geom, kSiteTileDims[c->site_tile][2], (size_t)4 * storage * c->wbytes, (size_t)24 << 20);
     c->geom.V = c->V;
     {   // K5 flavour: 0 = thread per (site, direction), 1 = thread per site (LGF_SITE_VARIANT / LGF_SITEMU_TILE: A/B knobs)
-        const char* e = getenv("LGF_SITE_VARIANT");
+        const char* e = knob("LGF_SITE_VARIANT");
         // measured at 32^4: the (site, direction) split wins for fp64 18-real and fp32 12-real
         // measured at 32^4: the shared-g (site, direction) kernel k5s wins for fp64 18-real (233 vs 247 us) and
         // fp32 12-real (102 vs 107 us); thread-per-site wins for fp64 12-real (175 vs 194 us) and fp32 18-real
         c->site_variant = e ? atoi(e) : 2;
         int t = (L[0] % 16 == 0) ? 2 : 0;
-        e = getenv("LGF_SITEMU_TILE");
+        e = knob("LGF_SITEMU_TILE");
         if (e && atoi(e) >= 0 && atoi(e) < kNumMuTiles) t = atoi(e);
         c->mu_tile = t;
         int n = 1;
@@ -932,7 +959,7 @@ static int create_common(const int32_t L[4], int precision, int storage, void* w
     set_walk(c->geom_mu, kMuTileDims[c->mu_tile][2], (size_t)8 * storage * c->wbytes);
     const int mu_default_fallback = ((precision == LGF_F64 && storage == LGF_REAL18) || (precision == LGF_F32 && storage == LGF_REAL12)) ? 0 : 1;
     {   // shared-g K5 (LGF_SITE_VARIANT=2, LGF_SITES_TILE): needs every extent to be a multiple of the tile's
-        const char* e = getenv("LGF_SITES_TILE");
+        const char* e = knob("LGF_SITES_TILE");
         int t = (e && atoi(e) >= 0 && atoi(e) < kNumSTiles) ? atoi(e) : (precision == LGF_F64 ? 2 : 3);
         for (int k = 0; k < 4 && !e; ++k)               // default tile does not divide the lattice: try the smallest one
             if (L[k] % kSTileDims[t][k]) { t = 0; break; }
@@ -962,7 +989,7 @@ static int create_common(const int32_t L[4], int precision, int storage, void* w
         if (e != cudaSuccess) rc = cuda_fail(e, "cudaStreamCreateWithFlags");
     }
     if (!rc) {
-        const char* e = getenv("LGF_DEFER_FINISH");
+        const char* e = knob("LGF_DEFER_FINISH");
         c->defer_finish = !(e && atoi(e) == 0);
         cudaError_t ce = cudaStreamCreateWithFlags(&c->fin_stream, cudaStreamNonBlocking);
         if (ce == cudaSuccess) ce = cudaEventCreateWithFlags(&c->ev_fork, cudaEventDisableTiming);
@@ -1022,8 +1049,12 @@ int lgf_destroy(lgf_ctx* c) {
     return LGF_OK;
 }
 
+// between lgf_iterate_async and lgf_wait the device owns the context's state: every other entry point refuses
+#define LGF_NOT_PENDING(c) do { if ((c)->pending_n >= 0) return LGF_ESTATE; } while (0)
+
 int lgf_load(lgf_ctx* c, const void* links, int memspace) {
     if (!c || !links || (memspace != LGF_HOST && memspace != LGF_DEVICE)) return LGF_EINVAL;
+    LGF_NOT_PENDING(c);
     const int rc = DISPATCH(c, load(c, links, memspace));
     if (rc) return rc;
     c->loaded = true;
@@ -1033,6 +1064,7 @@ int lgf_load(lgf_ctx* c, const void* links, int memspace) {
 
 int lgf_store(lgf_ctx* c, void* links, int memspace) {
     if (!c || !links || (memspace != LGF_HOST && memspace != LGF_DEVICE)) return LGF_EINVAL;
+    LGF_NOT_PENDING(c);
     if (!c->loaded) return LGF_ESTATE;
     return DISPATCH(c, store(c, links, memspace));
 }
@@ -1054,6 +1086,7 @@ static int finish(lgf_ctx* c, lgf_result* out, bool fix_mode) {
 
 int lgf_measure(lgf_ctx* c, lgf_result* out) {
     if (!c || !out) return LGF_EINVAL;
+    LGF_NOT_PENDING(c);
     if (!c->loaded) return LGF_ESTATE;
     int rc = init_state(c, -1.0, 0);
     if (!rc) rc = DISPATCH(c, k1(c, 0));
@@ -1070,6 +1103,7 @@ int lgf_measure(lgf_ctx* c, lgf_result* out) {
 
 int lgf_iterate_async(lgf_ctx* c, int64_t n, double alpha) {
     if (!c || n < 0 || !(alpha > 0)) return LGF_EINVAL;
+    LGF_NOT_PENDING(c);
     if (!c->loaded) return LGF_ESTATE;
     int rc = ensure_graph(c, alpha);
     if (!rc) rc = init_state(c, -1.0, (long long)n);
@@ -1100,6 +1134,7 @@ int lgf_iterate(lgf_ctx* c, int64_t n, double alpha, lgf_result* out) {
 
 int lgf_fix(lgf_ctx* c, double alpha, double theta_tol, int64_t max_iter, lgf_result* out) {
     if (!c || !out || !(alpha > 0) || max_iter < 0 || !(theta_tol == theta_tol)) return LGF_EINVAL;
+    LGF_NOT_PENDING(c);
     if (!c->loaded) return LGF_ESTATE;
     int rc = ensure_graph(c, alpha);
     if (!rc) rc = init_state(c, theta_tol, (long long)max_iter);
@@ -1144,12 +1179,14 @@ int lgf_fix(lgf_ctx* c, double alpha, double theta_tol, int64_t max_iter, lgf_re
 
 int lgf_debug_get_delta(lgf_ctx* c, void* delta_packed, int memspace) {
     if (!c || !delta_packed || (memspace != LGF_HOST && memspace != LGF_DEVICE)) return LGF_EINVAL;
+    LGF_NOT_PENDING(c);
     if (!c->loaded) return LGF_ESTATE;
     return DISPATCH(c, get_delta(c, delta_packed, memspace));
 }
 
 int lgf_debug_fourier_accelerate(lgf_ctx* c) {
     if (!c) return LGF_EINVAL;
+    LGF_NOT_PENDING(c);
     if (!c->loaded || !c->delta_valid) return LGF_ESTATE;
     int rc;
     for (int k = 0; k < 3; ++k)
@@ -1162,6 +1199,7 @@ int lgf_debug_fourier_accelerate(lgf_ctx* c) {
 
 int lgf_profile_iterate(lgf_ctx* c, int64_t n, double alpha, double ms[5], lgf_result* out) {
     if (!c || !ms || n <= 0 || !(alpha > 0)) return LGF_EINVAL;
+    LGF_NOT_PENDING(c);
     if (!c->loaded) return LGF_ESTATE;
     int rc = init_state(c, -1.0, (long long)n);
     if (!rc && !c->delta_valid) rc = DISPATCH(c, k1(c, 0));

@@ -11,8 +11,12 @@ static const ZtCtEntry* zt_tab(int precision, int* n) { return precision ? zt_ta
 
 // Several entries may serve the same extents (different splits / tile sizes): the first one is the
 // tuned default; LGF_XY_VARIANT / LGF_ZT_VARIANT = v select the v-th match (developer A/B knob).
+static const char* knob(const char* name) {       // developer knobs are honoured only with LGF_DEVKNOBS=1 (see lgf_api.cu)
+    const char* on = getenv("LGF_DEVKNOBS");
+    return (on && atoi(on) != 0) ? getenv(name) : nullptr;
+}
 static int variant(const char* name) {
-    const char* e = getenv(name);
+    const char* e = knob(name);
     return e ? atoi(e) : 0;
 }
 
@@ -64,9 +68,9 @@ static const ZtPipeEntry* ztp_tab(int precision, int* n) { return precision ? zt
 // K4 may run on a different tile shape than K2 (both read and write the natural layout on their own):
 // LGF_XYP_INV_VARIANT = v picks the v-th match; default: the same entry as K2 unless a tuned default exists.
 const XyPipeEntry* find_xy_pipe_inv(int precision, int nx, int ny, const XyPipeEntry* fwd) {
-    const char* e = getenv("LGF_XYP_INV_VARIANT");
+    const char* e = knob("LGF_XYP_INV_VARIANT");
     // measured: 48x48 fp32 planes run the inverse pass faster on 1-plane tiles (K4 24.9 -> 22.9 us at 48^3 x 8)
-    int skip = e ? atoi(e) : ((precision == 0 && nx == 48 && ny == 48 && !getenv("LGF_XYP_VARIANT")) ? 1 : -1);
+    int skip = e ? atoi(e) : ((precision == 0 && nx == 48 && ny == 48 && !knob("LGF_XYP_VARIANT")) ? 1 : -1);
     if (skip < 0 && fwd->k_inv) return fwd;
     if (skip < 0) skip = 0;                        // a forward-only entry (fft_xy_pipe_io): the first entry that has an inverse kernel
     int n = 0;

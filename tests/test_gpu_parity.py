@@ -316,6 +316,7 @@ def test_generic_and_compile_time_fft_paths_agree(monkeypatch):
     ref, thh, _ = oracle.iterate(L, U, 2, ALPHA)
     for force in (False, True):
         if force:
+            monkeypatch.setenv("LGF_DEVKNOBS", "1")
             monkeypatch.setenv("LGF_FORCE_GENERIC_FFT", "1")
         gf = _fixer(L, lgf.LGF_F64, lgf.LGF_REAL18, U)
         gf.iterate(2, ALPHA)
@@ -328,6 +329,7 @@ def test_generic_and_compile_time_fft_paths_agree(monkeypatch):
 def test_zblock_walk_order(monkeypatch, L, zb):
     """The site kernels' z-blocked (z-block outer, t inner) CTA order used on lattices whose t-slice outgrows
     the L2 (LGF_ZBLOCK forces it on small ones): same links, theta and F as the oracle, in every mode."""
+    monkeypatch.setenv("LGF_DEVKNOBS", "1")
     monkeypatch.setenv("LGF_ZBLOCK", zb)
     U = gi.make_config(L, 37, 0.59)
     ref, thh, Fh = oracle.iterate(L, U, 2, ALPHA)
@@ -353,6 +355,7 @@ def test_zblock_walk_order(monkeypatch, L, zb):
 def test_fused_update_kernel(monkeypatch, L, prec, stor):
     """K5 + K1 fused into the marching kernel (LGF_FUSED=1): out-of-place update with swapped link
     buffers; links after 1, 2 (odd/even buffer) and 5 iterations, theta/F and the fix count vs the oracle."""
+    monkeypatch.setenv("LGF_DEVKNOBS", "1")
     monkeypatch.setenv("LGF_FUSED", "1")
     U = gi.make_config(L, 31, 0.59)
     gf = _fixer(L, prec, stor, U)

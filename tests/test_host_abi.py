@@ -21,20 +21,23 @@ def test_workspace_bytes_host_logic():
     b18 = lgf.workspace_bytes((32, 32, 32, 32), lgf.LGF_F64, lgf.LGF_REAL18)
     b12 = lgf.workspace_bytes((32, 32, 32, 32), lgf.LGF_F64, lgf.LGF_REAL12)
     f18 = lgf.workspace_bytes((32, 32, 32, 32), lgf.LGF_F32, lgf.LGF_REAL18)
-    assert b18 - b12 == 2 * 4 * 6 * V * 8                  # 6 reals per link saved, in both link buffers
-    assert b18 >= 2 * 4 * 18 * V * 8 + 3 * 8 * V * 8       # two link buffers + Delta, Delta~, layout-B spectrum
+    assert b18 - b12 == 4 * 6 * V * 8                      # 6 reals per link saved
+    assert 4 * 18 * V * 8 + 2 * 8 * V * 8 <= b18 < 4 * 18 * V * 8 + 2.4 * 8 * V * 8   # links + Delta + padded layout-B spectrum + 19 MB staging
     assert f18 < b18
     assert lgf.workspace_bytes((5, 8, 8, 8), lgf.LGF_F64, lgf.LGF_REAL18) == 0     # 5 is not 2^a 3^b
     assert lgf.workspace_bytes((1, 8, 8, 8), lgf.LGF_F64, lgf.LGF_REAL18) == 0
     assert lgf.workspace_bytes((8, 8, 8, 8), 7, lgf.LGF_REAL18) == 0
     assert lgf.workspace_bytes((8, 8, 8, 8), lgf.LGF_F64, 10) == 0
     assert lgf.workspace_bytes((48, 48, 48, 8), lgf.LGF_F64, lgf.LGF_REAL12) > 0
+    assert lgf.workspace_bytes((4096, 4096, 2, 2), lgf.LGF_F64, lgf.LGF_REAL12) == 0      # V < 2^31, (x,y) plane too large for a tile
+    assert lgf.workspace_bytes((512, 512, 2, 2), lgf.LGF_F64, lgf.LGF_REAL12) == 0        # factorises, but no tile fits on chip
 
 
 def test_strerror_and_null_handling():
     lib = lgf.load_library()
     assert lib.lgf_strerror(0) == b"ok"
     assert b"invalid" in lib.lgf_strerror(-1)
+    assert b"host allocation" in lib.lgf_strerror(-5)
     assert lib.lgf_destroy(None) == -1
     assert lib.lgf_launch_count(None) == 0
     h = ctypes.c_void_p()
