@@ -112,6 +112,18 @@ int lgf_wait(lgf_ctx* ctx, lgf_result* out);
  * Reaching max_iter is not an error (converged = 0). */
 int lgf_fix(lgf_ctx* ctx, double alpha, double theta_tol, int64_t max_iter, lgf_result* out);
 
+/* The step after the path (eq. (1): "e^{-F_singlet(r,T)/T + C} = (1/3) <Tr(W(r) W^+(0))>, where W(.) is the
+ * temporal Wilson line"), evaluated on the links the context holds -- normally after lgf_fix, the quantity is not gauge
+ * invariant.  For ONE configuration the average <.> is the average over the spatial lattice, Vs = Lx*Ly*Lz sites
+ * xs = x + Lx*(y + Ly*z); the ensemble average and the fits of PAPER.md:78-80 are the caller's.
+ *   lgf_wilson_lines:       lines[xs][row][col][re,im] = U_t(xs,0) U_t(xs,1) ... U_t(xs,Lt-1)   (9 Vs complex, ordered product)
+ *   lgf_singlet_correlator: corr[r][re,im] = (1/(3 Vs)) sum_xs Tr[ W(xs + r) W(xs)^+ ], r = rx + Lx*(ry + Ly*rz), periodic
+ *                           (Vs complex; corr[0] = 1, corr[-r] = conj corr[r])
+ * Element type = ctx precision; host or device pointer per `memspace`; synchronous.  Both use the Delta fields as
+ * scratch (the next lgf_iterate re-measures first); theta, F and the links are untouched. */
+int lgf_wilson_lines(lgf_ctx* ctx, void* lines, int memspace);
+int lgf_singlet_correlator(lgf_ctx* ctx, void* corr, int memspace);
+
 /* Test/inspection hooks (device -> caller copies of intermediate fields of the LAST step executed):
  * the packed Delta field as [V][4] complex (c0 = D01, c1 = D02, c2 = D12, c3 = Im D00 + i Im D11),
  * element type = ctx precision.  After lgf_measure/lgf_iterate it holds Delta of the current links. */

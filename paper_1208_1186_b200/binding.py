@@ -71,6 +71,8 @@ def load_library() -> ctypes.CDLL:
     lib.lgf_fix.argtypes = [vp, ctypes.c_double, ctypes.c_double, ctypes.c_int64, rp]
     lib.lgf_profile_iterate.argtypes = [vp, ctypes.c_int64, ctypes.c_double, ctypes.POINTER(ctypes.c_double), rp]
     lib.lgf_debug_get_delta.argtypes = [vp, vp, ctypes.c_int]
+    lib.lgf_wilson_lines.argtypes = [vp, vp, ctypes.c_int]
+    lib.lgf_singlet_correlator.argtypes = [vp, vp, ctypes.c_int]
     lib.lgf_debug_fourier_accelerate.argtypes = [vp]
     lib.lgf_path_info.argtypes = [vp, i32p]
     lib.lgf_launch_count.restype = ctypes.c_int64
@@ -206,6 +208,22 @@ class GaugeFixer:
             _check(self.lib.lgf_profile_iterate(self._h, int(n), float(alpha), ms, ctypes.byref(r)), "lgf_profile_iterate")
         names = self.KERNELS_FUSED if self.path_info()["fused"] else self.KERNELS
         return {k: float(ms[i]) for i, k in enumerate(names)}, self._res(r)
+
+    def wilson_lines(self, device=None):
+        """Temporal Wilson lines of the current links: real tensor [Vs, 3, 3, 2]."""
+        out = self._torch.empty(self.V // self.L[3], 3, 3, 2, dtype=self.dtype, device=device or "cpu")
+        p, sp = self._ptr_space(out)
+        with self._torch.cuda.device(self.device):
+            _check(self.lib.lgf_wilson_lines(self._h, p, sp), "lgf_wilson_lines")
+        return out
+
+    def singlet_correlator(self, device=None):
+        """C(r) = (1/(3 Vs)) sum_x Tr[W(x + r) W(x)^+] of the current links: real tensor [Vs, 2], r with x fastest."""
+        out = self._torch.empty(self.V // self.L[3], 2, dtype=self.dtype, device=device or "cpu")
+        p, sp = self._ptr_space(out)
+        with self._torch.cuda.device(self.device):
+            _check(self.lib.lgf_singlet_correlator(self._h, p, sp), "lgf_singlet_correlator")
+        return out
 
     def debug_delta(self):
         """Packed Delta field as a host tensor [V,4,2]."""

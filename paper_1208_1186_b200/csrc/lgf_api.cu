@@ -21,6 +21,7 @@
 #include "lgf_site.cuh"
 #include "lgf_site_mu.cuh"
 #include "lgf_site_fused.cuh"
+#include "lgf_wilson.cuh"
 
 using namespace lgf;
 
@@ -771,6 +772,53 @@ struct Impl {
         CU(cudaStreamSynchronize(c->stream));
         return LGF_OK;
     }
+    // ---- the step after the path: temporal Wilson lines and the singlet correlator (lgf_wilson.cuh) ----
+    // scratch: the two Delta-sized fields (>= 8 V complex >= 11 Vs for Lt >= 2): W (9 Vs), P (Vs), G (Vs)
+    static Cx<T>* scratch(lgf_ctx* c) { return reinterpret_cast<Cx<T>*>(c->ws + c->lo.delta); }
+    static int lines(lgf_ctx* c) {
+        const long long Vs = c->V / c->L[3];
+        const int thr = 128;
+        k_wilson_lines<T, NC><<<(unsigned)((Vs + thr - 1) / thr), thr, 0, c->stream>>>(links(c), scratch(c), c->V, Vs, c->L[3]);
+        c->launches++;
+        CU(cudaGetLastError());
+        return LGF_OK;
+    }
+    static int wilson_lines_out(lgf_ctx* c, void* dst, int memspace) {
+        const long long Vs = c->V / c->L[3];
+        int rc = lines(c);
+        if (rc) return rc;
+        Cx<T>* aos = memspace == LGF_DEVICE ? reinterpret_cast<Cx<T>*>(dst) : scratch(c) + (size_t)9 * Vs;
+        k_lines_to_aos<T><<<(unsigned)((Vs * 9 + 255) / 256), 256, 0, c->stream>>>(scratch(c), aos, Vs);
+        c->launches++;
+        CU(cudaGetLastError());
+        if (memspace == LGF_HOST) CU(cudaMemcpyAsync(dst, aos, (size_t)9 * Vs * sizeof(Cx<T>), cudaMemcpyDeviceToHost, c->stream));
+        CU(cudaStreamSynchronize(c->stream));
+        return LGF_OK;
+    }
+    static int correlator(lgf_ctx* c, void* dst, int memspace) {
+        const long long Vs = c->V / c->L[3], LxLy = (long long)c->L[0] * c->L[1];
+        const int Lz = c->L[2], thr = 128;
+        int rc = lines(c);
+        if (rc) return rc;
+        Cx<T>* W = scratch(c);
+        Cx<T>* P = W + (size_t)9 * Vs;
+        Cx<T>* G = P + (size_t)Vs;
+        const int* nodone = nullptr;
+        launch_ex(c, fft_xy_kernel<T, -1>, dim3((unsigned)(9 * Lz)), dim3(c->xy_threads), c->xy_smem, W, c->xy, nodone);
+        const Cx<T>* twz = reinterpret_cast<const Cx<T>*>(c->axis[2].tw_fwd);
+        const Cx<T>* twzi = reinterpret_cast<const Cx<T>*>(c->axis[2].tw_inv);
+        k_z_power<T><<<(unsigned)((Vs + thr - 1) / thr), thr, 0, c->stream>>>(W, P, twz, LxLy, Lz);
+        k_z_inverse<T><<<(unsigned)((Vs + thr - 1) / thr), thr, 0, c->stream>>>(P, G, twzi, LxLy, Lz);
+        launch_ex(c, fft_xy_kernel<T, +1>, dim3((unsigned)Lz), dim3(c->xy_threads), c->xy_smem, G, c->xy, nodone);
+        Cx<T>* out = memspace == LGF_DEVICE ? reinterpret_cast<Cx<T>*>(dst) : P;
+        const T scale = (T)(1.0 / (3.0 * (double)Vs * (double)Vs));
+        k_corr_scale<T><<<(unsigned)((Vs + 255) / 256), 256, 0, c->stream>>>(G, out, Vs, scale);
+        c->launches += 5;
+        CU(cudaGetLastError());
+        if (memspace == LGF_HOST) CU(cudaMemcpyAsync(dst, out, (size_t)Vs * sizeof(Cx<T>), cudaMemcpyDeviceToHost, c->stream));
+        CU(cudaStreamSynchronize(c->stream));
+        return LGF_OK;
+    }
     static int get_delta(lgf_ctx* c, void* dst, int memspace) {
         const long long V = c->V;
         const int thr = 256;
@@ -1175,6 +1223,22 @@ int lgf_fix(lgf_ctx* c, double alpha, double theta_tol, int64_t max_iter, lgf_re
         slot ^= 1;
     }
     return finish(c, out, true);
+}
+
+int lgf_wilson_lines(lgf_ctx* c, void* lines, int memspace) {
+    if (!c || !lines || (memspace != LGF_HOST && memspace != LGF_DEVICE)) return LGF_EINVAL;
+    LGF_NOT_PENDING(c);
+    if (!c->loaded) return LGF_ESTATE;
+    c->delta_valid = false;             // the Delta fields serve as scratch
+    return DISPATCH(c, wilson_lines_out(c, lines, memspace));
+}
+
+int lgf_singlet_correlator(lgf_ctx* c, void* corr, int memspace) {
+    if (!c || !corr || (memspace != LGF_HOST && memspace != LGF_DEVICE)) return LGF_EINVAL;
+    LGF_NOT_PENDING(c);
+    if (!c->loaded) return LGF_ESTATE;
+    c->delta_valid = false;
+    return DISPATCH(c, correlator(c, corr, memspace));
 }
 
 int lgf_debug_get_delta(lgf_ctx* c, void* delta_packed, int memspace) {

@@ -518,3 +518,42 @@ def test_iterate_after_fix_without_reload(L):
     rb = gf2.iterate(3, ALPHA)
     assert ra.theta == rb.theta and ra.F == rb.F and torch.equal(after, gf2.store())
     gf2.close()
+
+
+@pytest.mark.parametrize("L", [(8, 8, 8, 8), (6, 4, 12, 8), (4, 6, 3, 2), (16, 16, 16, 4), (24, 18, 4, 8), (32, 32, 32, 8)])
+def test_wilson_lines_and_singlet_correlator(L):
+    """The step after the path (eq. (1)): Wilson lines and the singlet correlator of the GPU's links against
+    the oracle's written-out definition on the same links, fp64 (12- and 18-real) and fp32; then the same after a fix,
+    on the gauge-fixed links of both sides; the links, theta and F of the context are untouched by the measurement."""
+    U = gi.make_config(L, 61, 0.59)
+    Wo = oracle.wilson_lines(L, U)
+    Co = oracle.singlet_correlator(L, U) if gi.volume(L) // L[3] <= 8192 else None
+    for prec, stor in MODES:
+        gf = _fixer(L, prec, stor, U)
+        W = torch.view_as_complex(gf.wilson_lines()).numpy()
+        assert np.max(np.abs(W - Wo)) <= 1e-13
+        if Co is not None:
+            C = torch.view_as_complex(gf.singlet_correlator()).numpy()
+            assert np.max(np.abs(C - Co)) <= 1e-13
+            Cd = torch.view_as_complex(gf.singlet_correlator(device="cuda")).cpu().numpy()
+            assert np.array_equal(C, Cd)
+        r0 = gf.measure()
+        r = gf.iterate(3, ALPHA)
+        C3 = torch.view_as_complex(gf.singlet_correlator()).numpy()
+        assert abs(C3[0] - 1) <= 1e-13 and np.max(np.abs(C3)) <= 1 + 1e-13
+        r1 = gf.iterate(1, ALPHA)                          # the scratch use did not disturb the iteration
+        ref, thh, Fh = oracle.iterate(L, U, 4, ALPHA)
+        assert abs(r1.theta - thh[4]) <= 1e-10 * thh[4] and np.max(np.abs(_cplx(gf.store()) - ref)) <= 1e-11
+        if Co is not None:
+            Cfix = oracle.singlet_correlator(L, gf.store())
+            assert np.max(np.abs(torch.view_as_complex(gf.singlet_correlator()).numpy() - Cfix)) <= 1e-13
+        gf.close()
+    U32 = gi.as_real(U, torch.float32)
+    gf = lgf.GaugeFixer(L, lgf.LGF_F32, lgf.LGF_REAL12)
+    gf.load(U32)
+    Wo32 = oracle.wilson_lines(L, gi.from_real(U32))
+    assert np.max(np.abs(torch.view_as_complex(gf.wilson_lines().to(torch.float64)).numpy() - Wo32)) <= 2e-5
+    if Co is not None:
+        Co32 = oracle.singlet_correlator(L, gi.from_real(U32))
+        assert np.max(np.abs(torch.view_as_complex(gf.singlet_correlator().to(torch.float64)).numpy() - Co32)) <= 2e-5
+    gf.close()
