@@ -365,6 +365,31 @@ def main():
                                           "modes": {f"{p}_{s}": r for (p, s), r in rx.items()}}
     clocks = sampler.stop() if sampler else None
 
+    # ---- launch-bound lattices: one at a time and batched per launch (lgf_create_batch) ----
+    small = {}
+    if args.lattices != "none" and rank == 0:
+        for Ls, nb in (((8, 8, 8, 8), 64), ((16, 16, 16, 16), 16)):
+            ent = {}
+            for B in (1, nb):
+                Ub = torch.cat([gi.as_real(gi.make_config(Ls, gi.CONFIG_SEED + 10 + b, 0.59, device=dev)) for b in range(B)], 0)
+                gf = lgf.GaugeFixer(Ls, lgf.LGF_F64, 12, device=str(dev), nbatch=B)
+                gf.load(Ub)
+                gf.iterate(20, ALPHA)
+                stream = torch.cuda.current_stream(dev)
+                e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+                torch.cuda.synchronize()
+                e0.record(stream)
+                gf.iterate_async(200, ALPHA)
+                e1.record(stream)
+                gf.wait()
+                torch.cuda.synchronize()
+                us = e0.elapsed_time(e1) * 1e3 / 200
+                ent["single" if B == 1 else f"batch_{B}"] = {
+                    "us_per_launch_set": us, "us_per_lattice_iteration": us / B, "lattice_iterations_per_s": B / (us * 1e-6)}
+                gf.close()
+                del gf, Ub
+            small[lattice_name(Ls) + " f64_12"] = ent
+
     # ---- CPU baseline: the oracle, bounded sample, rank 0 at N = 1 only ----
     cpu = None
     if rank == 0 and world == 1 and not args.no_cpu_baseline:
@@ -402,6 +427,7 @@ def main():
             "clocks": clocks,
             "modes": {f"{p}_{s}": {k: v for k, v in r.items()} for (p, s), r in results.items()},
             "lattices": lattices,
+            "small_lattices": small,
         }
         print(json.dumps(line), flush=True)
     if world > 1:

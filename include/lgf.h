@@ -84,6 +84,20 @@ int lgf_create(const int32_t L[4], int precision, int storage, void* workspace_d
  * lgf_destroy) and uses the default stream.  For C callers and tests. */
 int lgf_create_simple(const int32_t L[4], int precision, int storage, lgf_ctx** out);
 
+/* Batched context ("batching many small lattices per launch"): `nbatch` independent lattices of
+ * the same shape, precision and storage are fixed by the SAME kernel launches (8^4 and 16^4 are launch-latency-bound
+ * one at a time).  Every link array passed to lgf_load / lgf_store then holds the nbatch lattices back to
+ * back (nbatch * V * 72 reals), and EVERY lgf_result pointer (lgf_measure, lgf_iterate, lgf_wait, lgf_fix,
+ * lgf_profile_iterate) must point to an array of nbatch results, one per lattice.  Each lattice has its own theta, F,
+ * iteration count and stopping test on the device: lgf_fix runs until every lattice has converged (or max_iter), and a
+ * lattice's links stop changing at ITS crossing, so its result is the one a single-lattice context gives.
+ * The inspection hooks and the Wilson-line calls are for single-lattice contexts (LGF_EUNSUPPORTED otherwise).
+ * nbatch * ceil(Lz/2) * Lt must not exceed 65535.  lgf_create(...) == lgf_create_batch(..., 1, ...). */
+size_t lgf_workspace_bytes_batch(const int32_t L[4], int precision, int storage, int32_t nbatch);
+int lgf_create_batch(const int32_t L[4], int precision, int storage, int32_t nbatch, void* workspace_dev,
+                     size_t workspace_bytes, void* cuda_stream, lgf_ctx** out);
+int32_t lgf_batch_size(const lgf_ctx* ctx);
+
 int lgf_destroy(lgf_ctx* ctx);
 
 /* Copy a link field in (boundary layout above, element type = ctx precision).  Synchronous with

@@ -61,6 +61,11 @@ def load_library() -> ctypes.CDLL:
     lib.lgf_workspace_bytes.argtypes = [i32p, ctypes.c_int, ctypes.c_int]
     lib.lgf_create.argtypes = [i32p, ctypes.c_int, ctypes.c_int, vp, ctypes.c_size_t, vp, ctypes.POINTER(vp)]
     lib.lgf_create_simple.argtypes = [i32p, ctypes.c_int, ctypes.c_int, ctypes.POINTER(vp)]
+    lib.lgf_workspace_bytes_batch.restype = ctypes.c_size_t
+    lib.lgf_workspace_bytes_batch.argtypes = [i32p, ctypes.c_int, ctypes.c_int, ctypes.c_int32]
+    lib.lgf_create_batch.argtypes = [i32p, ctypes.c_int, ctypes.c_int, ctypes.c_int32, vp, ctypes.c_size_t, vp, ctypes.POINTER(vp)]
+    lib.lgf_batch_size.restype = ctypes.c_int32
+    lib.lgf_batch_size.argtypes = [vp]
     lib.lgf_destroy.argtypes = [vp]
     lib.lgf_load.argtypes = [vp, vp, ctypes.c_int]
     lib.lgf_store.argtypes = [vp, vp, ctypes.c_int]
@@ -88,8 +93,8 @@ def _L(L: Sequence[int]):
     return (ctypes.c_int32 * 4)(*[int(v) for v in L])
 
 
-def workspace_bytes(L: Sequence[int], precision: int, storage: int) -> int:
-    return int(load_library().lgf_workspace_bytes(_L(L), precision, storage))
+def workspace_bytes(L: Sequence[int], precision: int, storage: int, nbatch: int = 1) -> int:
+    return int(load_library().lgf_workspace_bytes_batch(_L(L), precision, storage, int(nbatch)))
 
 
 def _check(rc: int, what: str) -> None:
@@ -99,10 +104,12 @@ def _check(rc: int, what: str) -> None:
 
 
 class GaugeFixer:
-    """One lattice on one GPU.  Methods mirror the C ABI: load, store, measure, iterate, fix."""
+    """One lattice -- or `nbatch` independent lattices of one shape fixed by the same launches -- on one GPU.  Methods
+    mirror the C ABI: load, store, measure, iterate, fix.  With nbatch > 1 link tensors carry a leading batch axis
+    ([nbatch * V, 4, 3, 3, 2]) and every result is a list of nbatch LgfResult."""
 
     def __init__(self, L: Sequence[int], precision: int = LGF_F64, storage: int = LGF_REAL18,
-                 device: str = "cuda:0", stream=None):
+                 device: str = "cuda:0", stream=None, nbatch: int = 1):
         import torch
         if not torch.cuda.is_available():
             raise LgfError("no CUDA device: the lgf library has no CPU fallback")
@@ -113,16 +120,17 @@ class GaugeFixer:
         self.precision, self.storage = precision, storage
         self.dtype = torch.float64 if precision == LGF_F64 else torch.float32
         self.device = torch.device(device)
-        nbytes = self.lib.lgf_workspace_bytes(_L(self.L), precision, storage)
+        self.nbatch = int(nbatch)
+        nbytes = self.lib.lgf_workspace_bytes_batch(_L(self.L), precision, storage, self.nbatch)
         if nbytes == 0:
-            raise LgfError(f"unsupported lattice {self.L} (extents must be 2^a 3^b >= 2)")
+            raise LgfError(f"unsupported lattice {self.L} x {self.nbatch} (extents must be 2^a 3^b >= 2, tiles must fit on chip)")
         with torch.cuda.device(self.device):
             self.workspace = torch.empty(nbytes + 256, dtype=torch.uint8, device=self.device)
             ptr = (self.workspace.data_ptr() + 255) // 256 * 256
             self.stream = stream if stream is not None else torch.cuda.current_stream(self.device)
             h = ctypes.c_void_p()
-            _check(self.lib.lgf_create(_L(self.L), precision, storage, ctypes.c_void_p(ptr), nbytes,
-                                       ctypes.c_void_p(self.stream.cuda_stream), ctypes.byref(h)), "lgf_create")
+            _check(self.lib.lgf_create_batch(_L(self.L), precision, storage, self.nbatch, ctypes.c_void_p(ptr), nbytes,
+                                             ctypes.c_void_p(self.stream.cuda_stream), ctypes.byref(h)), "lgf_create_batch")
         self._h = h
 
     def close(self) -> None:
@@ -143,7 +151,7 @@ class GaugeFixer:
 
     def load(self, links) -> None:
         """links: real tensor [V,4,3,3,2] (host or device) of the context precision."""
-        assert links.numel() == self.V * 72
+        assert links.numel() == self.nbatch * self.V * 72
         p, sp = self._ptr_space(links)
         with self._torch.cuda.device(self.device):
             _check(self.lib.lgf_load(self._h, p, sp), "lgf_load")
@@ -151,26 +159,29 @@ class GaugeFixer:
     def store(self, out=None, device=None):
         torch = self._torch
         if out is None:
-            out = torch.empty(self.V, 4, 3, 3, 2, dtype=self.dtype, device=device or "cpu")
+            out = torch.empty(self.nbatch * self.V, 4, 3, 3, 2, dtype=self.dtype, device=device or "cpu")
         p, sp = self._ptr_space(out)
         with torch.cuda.device(self.device):
             _check(self.lib.lgf_store(self._h, p, sp), "lgf_store")
         return out
 
-    @staticmethod
-    def _res(r: _Result) -> LgfResult:
-        return LgfResult(int(r.iterations), float(r.theta), float(r.F), bool(r.converged))
+    def _new_res(self):
+        return (_Result * self.nbatch)()
+
+    def _res(self, r):
+        out = [LgfResult(int(x.iterations), float(x.theta), float(x.F), bool(x.converged)) for x in r]
+        return out[0] if self.nbatch == 1 else out
 
     def measure(self) -> LgfResult:
-        r = _Result()
+        r = self._new_res()
         with self._torch.cuda.device(self.device):
-            _check(self.lib.lgf_measure(self._h, ctypes.byref(r)), "lgf_measure")
+            _check(self.lib.lgf_measure(self._h, r), "lgf_measure")
         return self._res(r)
 
     def iterate(self, n: int, alpha: float) -> LgfResult:
-        r = _Result()
+        r = self._new_res()
         with self._torch.cuda.device(self.device):
-            _check(self.lib.lgf_iterate(self._h, int(n), float(alpha), ctypes.byref(r)), "lgf_iterate")
+            _check(self.lib.lgf_iterate(self._h, int(n), float(alpha), r), "lgf_iterate")
         return self._res(r)
 
     def iterate_async(self, n: int, alpha: float) -> None:
@@ -178,15 +189,15 @@ class GaugeFixer:
             _check(self.lib.lgf_iterate_async(self._h, int(n), float(alpha)), "lgf_iterate_async")
 
     def wait(self) -> LgfResult:
-        r = _Result()
+        r = self._new_res()
         with self._torch.cuda.device(self.device):
-            _check(self.lib.lgf_wait(self._h, ctypes.byref(r)), "lgf_wait")
+            _check(self.lib.lgf_wait(self._h, r), "lgf_wait")
         return self._res(r)
 
     def fix(self, alpha: float, theta_tol: float, max_iter: int) -> LgfResult:
-        r = _Result()
+        r = self._new_res()
         with self._torch.cuda.device(self.device):
-            _check(self.lib.lgf_fix(self._h, float(alpha), float(theta_tol), int(max_iter), ctypes.byref(r)), "lgf_fix")
+            _check(self.lib.lgf_fix(self._h, float(alpha), float(theta_tol), int(max_iter), r), "lgf_fix")
         return self._res(r)
 
     KERNELS = ("K2_fft_xy_fwd", "K3_fft_zt_fwd_scale_inv", "K4_fft_xy_inv", "K5_gbuild_update", "K1_delta_theta_F")
@@ -203,9 +214,9 @@ class GaugeFixer:
         """-> (dict kernel name -> average ms per launch, LgfResult).  With the fused update kernel the
         dict has four entries (K5 and K1 are one kernel)."""
         ms = (ctypes.c_double * 5)()
-        r = _Result()
+        r = self._new_res()
         with self._torch.cuda.device(self.device):
-            _check(self.lib.lgf_profile_iterate(self._h, int(n), float(alpha), ms, ctypes.byref(r)), "lgf_profile_iterate")
+            _check(self.lib.lgf_profile_iterate(self._h, int(n), float(alpha), ms, r), "lgf_profile_iterate")
         names = self.KERNELS_FUSED if self.path_info()["fused"] else self.KERNELS
         return {k: float(ms[i]) for i, k in enumerate(names)}, self._res(r)
 

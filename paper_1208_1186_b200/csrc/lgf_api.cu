@@ -111,7 +111,7 @@ bool valid_args(const int32_t L[4], int precision, int storage) {
     return V < (1ll << 31);      // the site kernels index sites with 32-bit integers
 }
 
-Layout make_layout(const int32_t L[4], int precision, int storage, bool fused) {
+Layout make_layout(const int32_t L[4], int precision, int storage, bool fused, int nbatch = 1) {
     Layout lo;
     const size_t w = precision == LGF_F64 ? 8 : 4;
     const size_t V = (size_t)L[0] * L[1] * L[2] * L[3];
@@ -131,18 +131,19 @@ Layout make_layout(const int32_t L[4], int precision, int storage, bool fused) {
     for (int i = 0; i < 4; ++i) lo.nbm[i] = 0;
     lo.nblocks_mu = 0;             // set at create
     size_t off = 0;
-    lo.state = off; off += align_up(sizeof(DevState));
-    lo.partials = off; off += align_up(nb * sizeof(double2));
+    const size_t B = (size_t)nbatch;      // every per-lattice region holds the B lattices of a batched context back to back
+    lo.state = off; off += align_up(B * sizeof(DevState));
+    lo.partials = off; off += align_up(B * nb * sizeof(double2));
     for (int i = 0; i < 4; ++i) { lo.tw[i] = off; off += align_up((size_t)L[i] * 2 * w); }
     for (int i = 0; i < 4; ++i) { lo.twi[i] = off; off += align_up((size_t)L[i] * 2 * w); }
     for (int i = 0; i < 4; ++i) { lo.psq[i] = off; off += align_up((size_t)L[i] * w); }
     // the fused update kernel (opt-in) writes the new field out of place into a second link buffer (DevState::cur)
-    lo.links_bytes = align_up(4 * (size_t)(storage / 2) * V * 2 * w);
+    lo.links_bytes = align_up(B * 4 * (size_t)(storage / 2) * V * 2 * w);
     lo.links = off; off += (fused ? 2 : 1) * lo.links_bytes;
-    lo.delta = off; off += align_up(4 * V * 2 * w);
+    lo.delta = off; off += align_up(B * 4 * V * 2 * w);
     // layout-B spectrum between K2 and K3 (pipelined FFT path): tiles padded by one z entry per t row
-    lo.delta2 = off; off += align_up(4 * (V / L[2]) * (size_t)(L[2] + 1) * 2 * w);
-    lo.delta3 = off; off += fused ? align_up(4 * V * 2 * w) : 0;   // Delta of the new links (fused path: K1/K51 out, K2 in)
+    lo.delta2 = off; off += align_up(B * 4 * (V / L[2]) * (size_t)(L[2] + 1) * 2 * w);
+    lo.delta3 = off; off += fused ? align_up(B * 4 * V * 2 * w) : 0;   // Delta of the new links (fused path: K1/K51 out, K2 in)
     const size_t stage_sites = V < (size_t)kStageSites ? V : (size_t)kStageSites;
     lo.staging = off; off += align_up(stage_sites * 36 * 2 * w);
     lo.total = off;
@@ -154,6 +155,7 @@ Layout make_layout(const int32_t L[4], int precision, int storage, bool fused) {
 struct lgf_ctx {
     int32_t L[4];
     int precision, storage;
+    int nbatch;                  // lattices per launch (1 unless created by lgf_create_batch)
     long long V;
     size_t wbytes;               // bytes per real
     char* ws;                    // device workspace
@@ -246,7 +248,8 @@ cudaError_t launch_exc(lgf_ctx* c, const void* kernel, dim3 grid, dim3 block, vo
 }
 
 // grid of the site kernels: (x tiles, y tiles, z tiles * t tiles); see split_zt()
-dim3 grid3(const Geom& g) { return dim3((unsigned)g.nb[0], (unsigned)g.nb[1], (unsigned)(g.nb[2] * g.nb[3])); }
+// (lattice b of a batched context: blockIdx.z = b * nzt + (z,t) tile)
+dim3 grid3(const Geom& g, int nbatch) { return dim3((unsigned)g.nb[0], (unsigned)g.nb[1], (unsigned)(g.nb[2] * g.nb[3] * nbatch)); }
 unsigned magic_of(int d) { return d > 1 ? (unsigned)((0x100000000ULL + (unsigned)d - 1) / (unsigned)d) : 0u; }
 // walk order of the site kernels' (z, t) tiles (Geom::zb): z-blocks of about 16 MB of link traffic per t step once
 // a whole t-slice of links no longer fits the L2 comfortably (LGF_ZBLOCK overrides: z-tiles per block, 0 = plain order)
@@ -264,12 +267,17 @@ void set_walk(Geom& g, int tz, size_t link_bytes_per_site, size_t slice_limit = 
     g.zb = zb;
     g.zb_magic = magic_of(zb);
     g.nb3_magic = magic_of(g.nb[3]);
+    g.nzt = g.nb[2] * g.nb[3];
+    g.nzt_magic = magic_of(g.nzt);
+    g.nblocks = g.nb[0] * g.nb[1] * g.nzt;
 }
 
 DevState* dev_state(lgf_ctx* c) { return reinterpret_cast<DevState*>(c->ws + c->lo.state); }
 
-__global__ void reset_cur_kernel(DevState* st) { st->cur = 0; }
+// (one thread per lattice of a batched context)
+__global__ void reset_cur_kernel(DevState* st) { st[threadIdx.x].cur = 0; }
 __global__ void init_state_kernel(DevState* st, double tol, long long max_iter) {
+    st += threadIdx.x;
     st->iter = 0;
     st->done = 0;
     st->ticket = 0;
@@ -279,6 +287,7 @@ __global__ void init_state_kernel(DevState* st, double tol, long long max_iter) 
 }
 // after the initial measurement of lgf_fix: already converged (or max_iter == 0)?
 __global__ void initial_test_kernel(DevState* st) {
+    st += threadIdx.x;
     if (st->theta < st->tol || st->max_iter <= 0) st->done = 1;
 }
 
@@ -362,13 +371,13 @@ bool plan_passes(lgf_ctx* c) {
     if (c->xy_ct) {
         c->xy_args.twx_fwd = c->axis[0].tw_fwd; c->xy_args.twx_inv = c->axis[0].tw_inv;
         c->xy_args.twy_fwd = c->axis[1].tw_fwd; c->xy_args.twy_inv = c->axis[1].tw_inv;
-        c->xy_args.nplanes = (int)(4 * LzLt);
+        c->xy_args.nplanes = (int)(4 * LzLt * c->nbatch);
     }
     if (c->xy_pipe) {
         XyPipeArgs& P = c->xyp_args;
         P.twx_fwd = c->axis[0].tw_fwd; P.twx_inv = c->axis[0].tw_inv;
         P.twy_fwd = c->axis[1].tw_fwd; P.twy_inv = c->axis[1].tw_inv;
-        P.nplanes = (int)(4 * LzLt);
+        P.nplanes = (int)(4 * LzLt * c->nbatch);
         P.planes_per_comp = (int)LzLt;
         P.nz = L[2];
         P.pt = c->zt_pipe->cx * (L[2] + 1);
@@ -392,6 +401,7 @@ bool plan_passes(lgf_ctx* c) {
         A.twt_fwd = c->axis[3].tw_fwd; A.twt_inv = c->axis[3].tw_inv;
         A.psq_x = c->axis[0].psq; A.psq_y = c->axis[1].psq; A.psq_z = c->axis[2].psq; A.psq_t = c->axis[3].psq;
         A.V = c->V;
+        A.nbatch = c->nbatch;
         A.LxLy = LxLy;
         A.Lx = L[0];
         A.tiles_per_comp = (int)(LxLy / (c->zt_pipe ? c->zt_pipe->cx : c->zt_ct->cx));
@@ -414,6 +424,7 @@ bool tiles_fit(const int32_t L[4], int precision) {
     t->precision = precision;
     t->V = (long long)L[0] * L[1] * L[2] * L[3];
     t->wbytes = precision == LGF_F64 ? 8 : 4;
+    t->nbatch = 1;
     const bool ok = plan_passes(t);
     delete t;
     return ok;
@@ -452,7 +463,7 @@ int make_pipe_maps(lgf_ctx* c) {
     const cuuint64_t cb = 2 * c->wbytes, LxLy = (cuuint64_t)c->L[0] * c->L[1], Nz = c->L[2], Nt = c->L[3];
     if (e->tstore == 1) {
         const cuuint64_t C = e->perm_c, D = e->perm_d;
-        const cuuint64_t dims[5] = {2 * LxLy, Nz, D, C, 4};
+        const cuuint64_t dims[5] = {2 * LxLy, Nz, D, C, (cuuint64_t)(4 * c->nbatch)};
         const cuuint64_t strides[4] = {LxLy * cb, LxLy * Nz * cb, D * LxLy * Nz * cb, (cuuint64_t)c->V * cb};
         const cuuint32_t box[5] = {(cuuint32_t)(2 * e->cx), (cuuint32_t)(Nz + 1), (cuuint32_t)(D / 4), (cuuint32_t)C, 1};
         const int rc = encode_map(c, &c->zt_omap, 5, c->ws + c->lo.delta, dims, strides, box);
@@ -460,7 +471,7 @@ int make_pipe_maps(lgf_ctx* c) {
     }
     if (c->xy_pipe->io) {
         const XyPipeArgs& P = c->xyp_args;
-        const cuuint64_t dims[4] = {(cuuint64_t)(2 * e->cx), Nz + 1, Nt, (cuuint64_t)(4 * P.chunks_per_comp)};
+        const cuuint64_t dims[4] = {(cuuint64_t)(2 * e->cx), Nz + 1, Nt, (cuuint64_t)(4 * c->nbatch) * P.chunks_per_comp};
         const cuuint64_t strides[3] = {(cuuint64_t)e->cx * cb, (cuuint64_t)P.pt * cb, (cuuint64_t)P.tile_elems * cb};
         const cuuint32_t box[4] = {(cuuint32_t)(2 * e->cx), 1, 1, (cuuint32_t)P.store_tiles};
         return encode_map(c, &c->xy_bmap, 4, c->ws + c->lo.delta2, dims, strides, box);
@@ -508,11 +519,11 @@ struct Impl {
 
     static int k1(lgf_ctx* c, int mode, bool with_finish = true) {
         double2* partials = reinterpret_cast<double2*>(c->ws + c->lo.partials);
-#define LGF_K1_CASE(ID, TILE) case ID: launch_ex(c, k1_delta_theta_F<T, NC, TILE>, grid3(c->geom), dim3(TILE::kThreads), 0, \
+#define LGF_K1_CASE(ID, TILE) case ID: launch_ex(c, k1_delta_theta_F<T, NC, TILE>, grid3(c->geom, c->nbatch), dim3(TILE::kThreads), 0, \
             links(c), delta_src(c), partials, dev_state(c), c->geom, mode); break;
         switch (c->site_tile) {
             LGF_K1_CASE(1, Tile1) LGF_K1_CASE(2, Tile2) LGF_K1_CASE(3, Tile3) LGF_K1_CASE(4, Tile4) LGF_K1_CASE(5, Tile5)
-            default: launch_ex(c, k1_delta_theta_F<T, NC, Tile0>, grid3(c->geom), dim3(Tile0::kThreads), 0,
+            default: launch_ex(c, k1_delta_theta_F<T, NC, Tile0>, grid3(c->geom, c->nbatch), dim3(Tile0::kThreads), 0,
                 links(c), delta_src(c), partials, dev_state(c), c->geom, mode);
         }
 #undef LGF_K1_CASE
@@ -523,7 +534,7 @@ struct Impl {
     // k1_finish on the context's stream (mode 3: deferred, see lgf_ctx::defer_finish)
     static int k1_reduce(lgf_ctx* c, int mode) {
         double2* partials = reinterpret_cast<double2*>(c->ws + c->lo.partials);
-        launch_ex(c, k1_finish, dim3(1), dim3(kFinishThreads), 0, partials, c->lo.nblocks_site, dev_state(c), (double)c->V, mode);
+        launch_ex(c, k1_finish, dim3(c->nbatch), dim3(kFinishThreads), 0, partials, c->lo.nblocks_site, dev_state(c), (double)c->V, mode);
         c->launches++;
         CU(cudaGetLastError());
         return LGF_OK;
@@ -568,7 +579,7 @@ struct Impl {
     // pick the marching tile for this lattice (LGF_FUSED = 0 disables the fused path, LGF_FUSED_TILE = i forces entry i)
     static int plan_fused(lgf_ctx* c) {
         c->fused_tile = -1;
-        if (!c->xy_pipe) return LGF_OK;                    // the fused path rides on the pipelined FFT buffers
+        if (!c->xy_pipe || c->nbatch > 1) return LGF_OK;   // the fused path rides on the pipelined FFT buffers; single lattices only
         if (!fused_requested()) return LGF_OK;             // opt-in (LGF_DEVKNOBS=1 LGF_FUSED=1) until it beats K5 + K1 everywhere
         const char* ft = knob("LGF_FUSED_TILE");
         const FusedEntry* tab = fused_entries();
@@ -606,11 +617,11 @@ struct Impl {
 #else
             constexpr int kS3 = sizeof(T) == 8 ? 3 : 4;
 #endif
-#define LGF_K5S_CASE(ID, TILE, MINB) case ID: launch_ex(c, k5s_gbuild_update<T, NC, TILE, MINB>, grid3(c->geom_s), dim3(TILE::kThreads), 0,  \
+#define LGF_K5S_CASE(ID, TILE, MINB) case ID: launch_ex(c, k5s_gbuild_update<T, NC, TILE, MINB>, grid3(c->geom_s, c->nbatch), dim3(TILE::kThreads), 0,  \
                 links(c), delta(c), dev_state(c), c->geom_s, (T)(0.5 * alpha)); break;
             switch (c->s_tile) {
                 LGF_K5S_CASE(1, TileS1, 1) LGF_K5S_CASE(2, TileS2, kS3) LGF_K5S_CASE(3, TileS3, kS3) LGF_K5S_CASE(4, TileS4, 1)
-                default: launch_ex(c, k5s_gbuild_update<T, NC, TileS0, 2>, grid3(c->geom_s), dim3(TileS0::kThreads), 0, 
+                default: launch_ex(c, k5s_gbuild_update<T, NC, TileS0, 2>, grid3(c->geom_s, c->nbatch), dim3(TileS0::kThreads), 0, 
                     links(c), delta(c), dev_state(c), c->geom_s, (T)(0.5 * alpha));
             }
 #undef LGF_K5S_CASE
@@ -619,11 +630,11 @@ struct Impl {
             return LGF_OK;
         }
         if (c->site_variant == 0) {
-#define LGF_K5M_CASE(ID, TILE) case ID: launch_ex(c, k5m_gbuild_update<T, NC, TILE>, grid3(c->geom_mu), dim3(TILE::kThreads), 0,  \
+#define LGF_K5M_CASE(ID, TILE) case ID: launch_ex(c, k5m_gbuild_update<T, NC, TILE>, grid3(c->geom_mu, c->nbatch), dim3(TILE::kThreads), 0,  \
                 links(c), delta(c), dev_state(c), c->geom_mu, (T)(0.5 * alpha)); break;
             switch (c->mu_tile) {
                 LGF_K5M_CASE(1, TileM1) LGF_K5M_CASE(2, TileM2)
-                default: launch_ex(c, k5m_gbuild_update<T, NC, TileM0>, grid3(c->geom_mu), dim3(TileM0::kThreads), 0, 
+                default: launch_ex(c, k5m_gbuild_update<T, NC, TileM0>, grid3(c->geom_mu, c->nbatch), dim3(TileM0::kThreads), 0, 
                     links(c), delta(c), dev_state(c), c->geom_mu, (T)(0.5 * alpha));
             }
 #undef LGF_K5M_CASE
@@ -631,11 +642,11 @@ struct Impl {
             CU(cudaGetLastError());
             return LGF_OK;
         }
-#define LGF_K5_CASE(ID, TILE) case ID: launch_ex(c, k5_gbuild_update<T, NC, TILE>, grid3(c->geom), dim3(TILE::kThreads), 0,  \
+#define LGF_K5_CASE(ID, TILE) case ID: launch_ex(c, k5_gbuild_update<T, NC, TILE>, grid3(c->geom, c->nbatch), dim3(TILE::kThreads), 0,  \
             links(c), delta(c), dev_state(c), c->geom, (T)(0.5 * alpha)); break;
         switch (c->site_tile) {
             LGF_K5_CASE(1, Tile1) LGF_K5_CASE(2, Tile2) LGF_K5_CASE(3, Tile3) LGF_K5_CASE(4, Tile4) LGF_K5_CASE(5, Tile5)
-            default: launch_ex(c, k5_gbuild_update<T, NC, Tile0>, grid3(c->geom), dim3(Tile0::kThreads), 0, 
+            default: launch_ex(c, k5_gbuild_update<T, NC, Tile0>, grid3(c->geom, c->nbatch), dim3(Tile0::kThreads), 0, 
                 links(c), delta(c), dev_state(c), c->geom, (T)(0.5 * alpha));
         }
 #undef LGF_K5_CASE
@@ -644,8 +655,9 @@ struct Impl {
         return LGF_OK;
     }
     static int fft(lgf_ctx* c, int k, bool gated) {
-        const int* done = gated ? &dev_state(c)->done : nullptr;
-        const unsigned planes = (unsigned)(4 * (long long)c->L[2] * c->L[3]);
+        // (batched contexts: the per-lattice `done` flags gate K5 and K1; the FFT passes run ungated)
+        const int* done = (gated && c->nbatch == 1) ? &dev_state(c)->done : nullptr;
+        const unsigned planes = (unsigned)(4 * (long long)c->L[2] * c->L[3] * c->nbatch);
         Cx<T>* dptr = delta(c);
         if (c->xy_pipe) {
             Cx<T>* d2 = reinterpret_cast<Cx<T>*>(c->ws + c->lo.delta2);
@@ -673,7 +685,7 @@ struct Impl {
         if (k == 1 && c->zt_ct) {
             const ZtCtEntry* e = c->zt_ct;
             void* args[] = {&dptr, &c->zt_args, &done};
-            CU(launch_exc(c, e->kernel, dim3(4 * c->zt_args.tiles_per_comp), dim3(e->threads), args, e->smem));
+            CU(launch_exc(c, e->kernel, dim3(4 * c->nbatch * c->zt_args.tiles_per_comp), dim3(e->threads), args, e->smem));
             c->launches++;
             return LGF_OK;
         }
@@ -682,7 +694,7 @@ struct Impl {
         else if (k == 2)
             launch_ex(c, fft_xy_kernel<T, +1>, dim3(planes), dim3(c->xy_threads), c->xy_smem, delta(c), c->xy, done);
         else
-            launch_ex(c, fft_zt_kernel<T>, dim3(4 * c->zt.tiles_per_comp), dim3(c->zt_threads), c->zt_smem, delta(c), c->zt, c->V, done);
+            launch_ex(c, fft_zt_kernel<T>, dim3(4 * c->nbatch * c->zt.tiles_per_comp), dim3(c->zt_threads), c->zt_smem, delta(c), c->zt, c->V, done);
         c->launches++;
         CU(cudaGetLastError());
         return LGF_OK;
@@ -705,7 +717,7 @@ struct Impl {
             CU(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, c->xy_pipe_inv->k_inv, c->xy_pipe_inv->threads, c->xy_pipe_inv->smem));
             if (occ < 1) return cuda_fail(cudaErrorLaunchOutOfResources, "fft_xy_pipe (inverse) does not fit on an SM");
             c->xyp_inv_grid = inv_tiles < occ * sms ? inv_tiles : occ * sms;
-            const int zt_tiles = 4 * c->zt_args.tiles_per_comp;
+            const int zt_tiles = 4 * c->nbatch * c->zt_args.tiles_per_comp;
             CU(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, c->zt_pipe->kernel, c->zt_pipe->threads, c->zt_pipe->smem));
             if (occ < 1) return cuda_fail(cudaErrorLaunchOutOfResources, "fft_zt_pipe does not fit on an SM");
             c->ztp_grid = zt_tiles < occ * sms ? zt_tiles : occ * sms;
@@ -724,25 +736,26 @@ struct Impl {
         const long long V = c->V;
         const int thr = 256;
         c->cur_host = 0;                                   // a fresh field always lands in buffer 0
-        reset_cur_kernel<<<1, 1, 0, c->stream>>>(dev_state(c));
+        reset_cur_kernel<<<1, c->nbatch, 0, c->stream>>>(dev_state(c));
         c->launches++;
         CU(cudaGetLastError());
-        if (memspace == LGF_DEVICE) {
-            const long long n = V * 36;
-            aos_to_soa<T, NC><<<(unsigned)((n + thr - 1) / thr), thr, 0, c->stream>>>(
-                reinterpret_cast<const Cx<T>*>(src), links(c), V, 0, V);
-            c->launches++;
-            CU(cudaGetLastError());
-        } else {
-            const char* h = reinterpret_cast<const char*>(src);
-            for (long long s0 = 0; s0 < V; s0 += kStageSites) {
-                const long long ns = (V - s0 < kStageSites) ? V - s0 : kStageSites;
-                CU(cudaMemcpyAsync(staging(c), h + (size_t)s0 * 36 * sizeof(Cx<T>), (size_t)ns * 36 * sizeof(Cx<T>),
-                                   cudaMemcpyHostToDevice, c->stream));
-                const long long n = ns * 36;
-                aos_to_soa<T, NC><<<(unsigned)((n + thr - 1) / thr), thr, 0, c->stream>>>(staging(c), links(c), V, s0, ns);
+        for (int b = 0; b < c->nbatch; ++b) {             // the lattices of a batched context lie back to back, here and there
+            Cx<T>* Ub = links(c) + (size_t)b * 4 * NC * V;
+            const Cx<T>* sb = reinterpret_cast<const Cx<T>*>(src) + (size_t)b * V * 36;
+            if (memspace == LGF_DEVICE) {
+                const long long n = V * 36;
+                aos_to_soa<T, NC><<<(unsigned)((n + thr - 1) / thr), thr, 0, c->stream>>>(sb, Ub, V, 0, V);
                 c->launches++;
                 CU(cudaGetLastError());
+            } else {
+                for (long long s0 = 0; s0 < V; s0 += kStageSites) {
+                    const long long ns = (V - s0 < kStageSites) ? V - s0 : kStageSites;
+                    CU(cudaMemcpyAsync(staging(c), sb + (size_t)s0 * 36, (size_t)ns * 36 * sizeof(Cx<T>), cudaMemcpyHostToDevice, c->stream));
+                    const long long n = ns * 36;
+                    aos_to_soa<T, NC><<<(unsigned)((n + thr - 1) / thr), thr, 0, c->stream>>>(staging(c), Ub, V, s0, ns);
+                    c->launches++;
+                    CU(cudaGetLastError());
+                }
             }
         }
         CU(cudaStreamSynchronize(c->stream));
@@ -751,22 +764,23 @@ struct Impl {
     static int store(lgf_ctx* c, void* dst, int memspace) {
         const long long V = c->V;
         const int thr = 256;
-        if (memspace == LGF_DEVICE) {
-            const long long n = V * 4;
-            soa_to_aos<T, NC><<<(unsigned)((n + thr - 1) / thr), thr, 0, c->stream>>>(
-                links(c), reinterpret_cast<Cx<T>*>(dst), V, 0, V);
-            c->launches++;
-            CU(cudaGetLastError());
-        } else {
-            char* h = reinterpret_cast<char*>(dst);
-            for (long long s0 = 0; s0 < V; s0 += kStageSites) {
-                const long long ns = (V - s0 < kStageSites) ? V - s0 : kStageSites;
-                const long long n = ns * 4;
-                soa_to_aos<T, NC><<<(unsigned)((n + thr - 1) / thr), thr, 0, c->stream>>>(links(c), staging(c), V, s0, ns);
+        for (int b = 0; b < c->nbatch; ++b) {
+            const Cx<T>* Ub = links(c) + (size_t)b * 4 * NC * V;
+            Cx<T>* db = reinterpret_cast<Cx<T>*>(dst) + (size_t)b * V * 36;
+            if (memspace == LGF_DEVICE) {
+                const long long n = V * 4;
+                soa_to_aos<T, NC><<<(unsigned)((n + thr - 1) / thr), thr, 0, c->stream>>>(Ub, db, V, 0, V);
                 c->launches++;
                 CU(cudaGetLastError());
-                CU(cudaMemcpyAsync(h + (size_t)s0 * 36 * sizeof(Cx<T>), staging(c), (size_t)ns * 36 * sizeof(Cx<T>),
-                                   cudaMemcpyDeviceToHost, c->stream));
+            } else {
+                for (long long s0 = 0; s0 < V; s0 += kStageSites) {
+                    const long long ns = (V - s0 < kStageSites) ? V - s0 : kStageSites;
+                    const long long n = ns * 4;
+                    soa_to_aos<T, NC><<<(unsigned)((n + thr - 1) / thr), thr, 0, c->stream>>>(Ub, staging(c), V, s0, ns);
+                    c->launches++;
+                    CU(cudaGetLastError());
+                    CU(cudaMemcpyAsync(db + (size_t)s0 * 36, staging(c), (size_t)ns * 36 * sizeof(Cx<T>), cudaMemcpyDeviceToHost, c->stream));
+                }
             }
         }
         CU(cudaStreamSynchronize(c->stream));
@@ -911,14 +925,14 @@ int enqueue_iterations(lgf_ctx* c, int64_t n) {
 }
 
 int init_state(lgf_ctx* c, double tol, long long max_iter) {
-    init_state_kernel<<<1, 1, 0, c->stream>>>(dev_state(c), tol, max_iter);
+    init_state_kernel<<<1, c->nbatch, 0, c->stream>>>(dev_state(c), tol, max_iter);
     c->launches++;
     CU(cudaGetLastError());
     return LGF_OK;
 }
 
 int fetch_state(lgf_ctx* c, int slot) {
-    CU(cudaMemcpyAsync(&c->host_state[slot], dev_state(c), sizeof(DevState), cudaMemcpyDeviceToHost, c->stream));
+    CU(cudaMemcpyAsync(&c->host_state[(size_t)slot * c->nbatch], dev_state(c), (size_t)c->nbatch * sizeof(DevState), cudaMemcpyDeviceToHost, c->stream));
     return LGF_OK;
 }
 
@@ -951,7 +965,7 @@ size_t lgf_workspace_bytes(const int32_t L[4], int precision, int storage) {
     return make_layout(L, precision, storage, fused_requested()).total;
 }
 
-static int create_common(const int32_t L[4], int precision, int storage, void* ws, size_t ws_bytes, bool owns,
+static int create_common(const int32_t L[4], int precision, int storage, int nbatch, void* ws, size_t ws_bytes, bool owns,
                          void* stream, lgf_ctx** out) {
     lgf_ctx* c = new (std::nothrow) lgf_ctx();
     if (!c) return LGF_ENOMEM;
@@ -959,12 +973,13 @@ static int create_common(const int32_t L[4], int precision, int storage, void* w
     for (int i = 0; i < 4; ++i) c->L[i] = L[i];
     c->precision = precision;
     c->storage = storage;
+    c->nbatch = nbatch;
     c->V = (long long)L[0] * L[1] * L[2] * L[3];
     c->wbytes = precision == LGF_F64 ? 8 : 4;
     c->ws = reinterpret_cast<char*>(ws);
     c->owns_ws = owns;
     c->stream = reinterpret_cast<cudaStream_t>(stream);
-    c->lo = make_layout(L, precision, storage, fused_requested());
+    c->lo = make_layout(L, precision, storage, fused_requested() && nbatch == 1, nbatch);
     c->pending_n = -1;
     {
         const char* e = knob("LGF_PDL");
@@ -1029,7 +1044,7 @@ static int create_common(const int32_t L[4], int precision, int storage, void* w
     if (ws_bytes < c->lo.total || (reinterpret_cast<uintptr_t>(ws) % kAlign) != 0) rc = LGF_EINVAL;
     if (!rc && !plan_passes(c)) rc = LGF_EUNSUPPORTED;
     if (!rc) {
-        cudaError_t e = cudaMallocHost(reinterpret_cast<void**>(&c->host_state), 2 * sizeof(DevState));
+        cudaError_t e = cudaMallocHost(reinterpret_cast<void**>(&c->host_state), 2 * (size_t)nbatch * sizeof(DevState));
         if (e != cudaSuccess) rc = cuda_fail(e, "cudaMallocHost");
     }
     if (!rc) {
@@ -1067,8 +1082,31 @@ int lgf_create(const int32_t L[4], int precision, int storage, void* workspace_d
                void* cuda_stream, lgf_ctx** out) {
     if (!out || !workspace_dev || !valid_args(L, precision, storage)) return LGF_EINVAL;
     if (lgf_workspace_bytes(L, precision, storage) == 0) return LGF_EUNSUPPORTED;
-    return create_common(L, precision, storage, workspace_dev, workspace_bytes, false, cuda_stream, out);
+    return create_common(L, precision, storage, 1, workspace_dev, workspace_bytes, false, cuda_stream, out);
 }
+
+static bool valid_batch(const int32_t L[4], int nbatch) {
+    // grid z = (z,t) tiles x lattices must stay below 2^16 for every site-kernel tiling (the smallest tile is 2 x 1 in z, t)
+    return nbatch >= 1 && (long long)nbatch * ((L[2] + 1) / 2) * L[3] <= 65535;
+}
+
+size_t lgf_workspace_bytes_batch(const int32_t L[4], int precision, int storage, int32_t nbatch) {
+    if (!valid_args(L, precision, storage) || !valid_batch(L, nbatch)) return 0;
+    Axis ax;
+    for (int i = 0; i < 4; ++i)
+        if (!factor23(L[i], &ax)) return 0;
+    if (!tiles_fit(L, precision)) return 0;
+    return make_layout(L, precision, storage, fused_requested() && nbatch == 1, nbatch).total;
+}
+
+int lgf_create_batch(const int32_t L[4], int precision, int storage, int32_t nbatch, void* workspace_dev, size_t workspace_bytes,
+                     void* cuda_stream, lgf_ctx** out) {
+    if (!out || !workspace_dev || !valid_args(L, precision, storage) || nbatch < 1) return LGF_EINVAL;
+    if (lgf_workspace_bytes_batch(L, precision, storage, nbatch) == 0) return LGF_EUNSUPPORTED;
+    return create_common(L, precision, storage, nbatch, workspace_dev, workspace_bytes, false, cuda_stream, out);
+}
+
+int32_t lgf_batch_size(const lgf_ctx* c) { return c ? c->nbatch : 0; }
 
 int lgf_create_simple(const int32_t L[4], int precision, int storage, lgf_ctx** out) {
     if (!out || !valid_args(L, precision, storage)) return LGF_EINVAL;
@@ -1076,7 +1114,7 @@ int lgf_create_simple(const int32_t L[4], int precision, int storage, lgf_ctx** 
     if (bytes == 0) return LGF_EUNSUPPORTED;
     void* ws = nullptr;
     CU(cudaMalloc(&ws, bytes));
-    const int rc = create_common(L, precision, storage, ws, bytes, true, nullptr, out);
+    const int rc = create_common(L, precision, storage, 1, ws, bytes, true, nullptr, out);
     if (rc) cudaFree(ws);
     return rc;
 }
@@ -1121,13 +1159,13 @@ static int finish(lgf_ctx* c, lgf_result* out, bool fix_mode) {
     int rc = fetch_state(c, 0);
     if (rc) return rc;
     CU(cudaStreamSynchronize(c->stream));
-    const DevState& s = c->host_state[0];
-    c->cur_host = s.cur;
-    if (out) {
-        out->iterations = s.iter;
-        out->theta = s.theta;
-        out->F = s.F;
-        out->converged = fix_mode ? (s.theta < s.tol ? 1 : 0) : 0;
+    c->cur_host = c->host_state[0].cur;
+    for (int b = 0; out && b < c->nbatch; ++b) {           // one result per lattice of a batched context
+        const DevState& s = c->host_state[b];
+        out[b].iterations = s.iter;
+        out[b].theta = s.theta;
+        out[b].F = s.F;
+        out[b].converged = fix_mode ? (s.theta < s.tol ? 1 : 0) : 0;
     }
     return LGF_OK;
 }
@@ -1141,11 +1179,10 @@ int lgf_measure(lgf_ctx* c, lgf_result* out) {
     if (rc) return rc;
     c->delta_valid = true;
     c->dbg_delta_tilde = false;
-    lgf_result r;
-    rc = finish(c, &r, false);
+    std::vector<lgf_result> r((size_t)c->nbatch);
+    rc = finish(c, r.data(), false);
     if (rc) return rc;
-    r.iterations = 0;
-    *out = r;
+    for (int b = 0; b < c->nbatch; ++b) { r[b].iterations = 0; out[b] = r[b]; }
     return LGF_OK;
 }
 
@@ -1165,11 +1202,11 @@ int lgf_iterate_async(lgf_ctx* c, int64_t n, double alpha) {
 int lgf_wait(lgf_ctx* c, lgf_result* out) {
     if (!c) return LGF_EINVAL;
     if (c->pending_n < 0) return LGF_ESTATE;
-    lgf_result r;
-    const int rc = finish(c, &r, false);
+    std::vector<lgf_result> r((size_t)c->nbatch);
+    const int rc = finish(c, r.data(), false);
     c->pending_n = -1;
     if (rc) return rc;
-    if (out) *out = r;
+    for (int b = 0; out && b < c->nbatch; ++b) out[b] = r[b];
     return LGF_OK;
 }
 
@@ -1190,7 +1227,7 @@ int lgf_fix(lgf_ctx* c, double alpha, double theta_tol, int64_t max_iter, lgf_re
     if (rc) return rc;
     c->delta_valid = true;
     c->dbg_delta_tilde = false;
-    initial_test_kernel<<<1, 1, 0, c->stream>>>(dev_state(c));
+    initial_test_kernel<<<1, c->nbatch, 0, c->stream>>>(dev_state(c));
     c->launches++;
     CU(cudaGetLastError());
     // Batches of kFixBatch gated iterations; the state block is copied to pinned memory after each
@@ -1211,7 +1248,9 @@ int lgf_fix(lgf_ctx* c, double alpha, double theta_tol, int64_t max_iter, lgf_re
         CU(cudaEventRecord(c->ev[slot], c->stream));
         if (have_prev) {
             CU(cudaEventSynchronize(c->ev[prev_slot]));
-            if (c->host_state[prev_slot].done) done = true;
+            bool all = true;                               // a batched context stops when every lattice has
+            for (int b = 0; b < c->nbatch; ++b) all = all && c->host_state[(size_t)prev_slot * c->nbatch + b].done;
+            if (all) done = true;
         }
         if (nb <= 0 || enq >= max_iter) {
             // nothing more to enqueue: drain the last batch
@@ -1222,7 +1261,12 @@ int lgf_fix(lgf_ctx* c, double alpha, double theta_tol, int64_t max_iter, lgf_re
         prev_slot = slot;
         slot ^= 1;
     }
-    return finish(c, out, true);
+    std::vector<lgf_result> r((size_t)c->nbatch);
+    rc = finish(c, r.data(), true);
+    if (rc) return rc;
+    for (int b = 0; b < c->nbatch; ++b) out[b] = r[b];
+    if (c->nbatch > 1) c->delta_valid = false;     // the ungated FFT passes of a batched context went on past each lattice's crossing
+    return LGF_OK;
 }
 
 int lgf_wilson_lines(lgf_ctx* c, void* lines, int memspace) {
@@ -1230,6 +1274,7 @@ int lgf_wilson_lines(lgf_ctx* c, void* lines, int memspace) {
     LGF_NOT_PENDING(c);
     if (!c->loaded) return LGF_ESTATE;
     c->delta_valid = false;             // the Delta fields serve as scratch
+    if (c->nbatch != 1) return LGF_EUNSUPPORTED;   // single-lattice contexts only
     return DISPATCH(c, wilson_lines_out(c, lines, memspace));
 }
 
@@ -1238,6 +1283,7 @@ int lgf_singlet_correlator(lgf_ctx* c, void* corr, int memspace) {
     LGF_NOT_PENDING(c);
     if (!c->loaded) return LGF_ESTATE;
     c->delta_valid = false;
+    if (c->nbatch != 1) return LGF_EUNSUPPORTED;   // single-lattice contexts only
     return DISPATCH(c, correlator(c, corr, memspace));
 }
 
@@ -1245,6 +1291,7 @@ int lgf_debug_get_delta(lgf_ctx* c, void* delta_packed, int memspace) {
     if (!c || !delta_packed || (memspace != LGF_HOST && memspace != LGF_DEVICE)) return LGF_EINVAL;
     LGF_NOT_PENDING(c);
     if (!c->loaded) return LGF_ESTATE;
+    if (c->nbatch != 1) return LGF_EUNSUPPORTED;   // single-lattice contexts only
     return DISPATCH(c, get_delta(c, delta_packed, memspace));
 }
 
@@ -1252,6 +1299,7 @@ int lgf_debug_fourier_accelerate(lgf_ctx* c) {
     if (!c) return LGF_EINVAL;
     LGF_NOT_PENDING(c);
     if (!c->loaded || !c->delta_valid) return LGF_ESTATE;
+    if (c->nbatch != 1) return LGF_EUNSUPPORTED;
     int rc;
     for (int k = 0; k < 3; ++k)
         if ((rc = DISPATCH(c, fft(c, k, false)))) return rc;
@@ -1293,10 +1341,10 @@ int lgf_profile_iterate(lgf_ctx* c, int64_t n, double alpha, double ms[5], lgf_r
     for (int i = 0; i < 6; ++i) cudaEventDestroy(ev[i]);
     if (rc) return rc;
     for (int k = 0; k < 5; ++k) ms[k] = acc[k] / (double)n;
-    lgf_result r;
-    rc = finish(c, &r, false);
+    std::vector<lgf_result> r((size_t)c->nbatch);
+    rc = finish(c, r.data(), false);
     if (rc) return rc;
-    if (out) *out = r;
+    for (int b = 0; out && b < c->nbatch; ++b) out[b] = r[b];
     return LGF_OK;
 }
 

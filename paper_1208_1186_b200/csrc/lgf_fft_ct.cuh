@@ -197,6 +197,7 @@ struct ZtArgs {
     long long LxLy;
     int Lx;
     int tiles_per_comp;               // LxLy / CX
+    int nbatch;                       // lattices per launch (batched contexts): components run over 4 * nbatch
     double scale_num;                 // p2max / V
     int x_n1, x_n2, y_n1, y_n2;       // how K2 split the x and y lines (digit-swapped spectrum order)
     // psq_t[k] for k = 0..Lt/2, by value (read as constant-bank operands by the whole-line t pass of the pipelined K3;

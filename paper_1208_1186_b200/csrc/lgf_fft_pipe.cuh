@@ -238,7 +238,7 @@ fft_zt_pipe(const Cx<T>* inB, Cx<T>* out, const ZtArgs A, const int* done) {
     Cx<T>* bufs = reinterpret_cast<Cx<T>*>(pipe_smem);
     uint64_t* full = reinterpret_cast<uint64_t*>(pipe_smem + sizeof(Cx<T>) * (size_t)NBUF * TILE);
     const int tid = threadIdx.x, g = tid / GT, gtid = tid - g * GT;
-    const int ntiles = 4 * A.tiles_per_comp;
+    const int ntiles = 4 * A.nbatch * A.tiles_per_comp;
     const int my_tiles = (int)blockIdx.x < ntiles ? (ntiles - (int)blockIdx.x + (int)gridDim.x - 1) / (int)gridDim.x : 0;
     const long long gz = A.LxLy, gt = A.LxLy * NZ;
     const Cx<T>* twz_f = reinterpret_cast<const Cx<T>*>(A.twz_fwd);

@@ -246,7 +246,7 @@ fft_zt_pipe3(const Cx<T>* inB, Cx<T>* out, const __grid_constant__ ZtArgs A, con
     Cx<T>* bufs = reinterpret_cast<Cx<T>*>(pipe_smem);
     uint64_t* full = reinterpret_cast<uint64_t*>(pipe_smem + sizeof(Cx<T>) * (size_t)NBUF * TILE);
     const int tid = threadIdx.x, g = tid / GT, gtid = tid - g * GT;
-    const int ntiles = 4 * A.tiles_per_comp;
+    const int ntiles = 4 * A.nbatch * A.tiles_per_comp;
     const int my_tiles = (int)blockIdx.x < ntiles ? (ntiles - (int)blockIdx.x + (int)gridDim.x - 1) / (int)gridDim.x : 0;
     const long long gz = A.LxLy, gt = A.LxLy * NZ;
 
@@ -328,7 +328,7 @@ fft_zt_pipe3q(const Cx<T>* inB, Cx<T>* out, const __grid_constant__ ZtArgs A, co
     uint64_t* full = reinterpret_cast<uint64_t*>(twt + D * (C - 1));
     const int tid = threadIdx.x;
     const bool io = tid == GT - 1;
-    const int ntiles = 4 * A.tiles_per_comp;
+    const int ntiles = 4 * A.nbatch * A.tiles_per_comp;
     const int my_tiles = (int)blockIdx.x < ntiles ? (ntiles - (int)blockIdx.x + (int)gridDim.x - 1) / (int)gridDim.x : 0;
 
     auto issue = [&](int k) {             // quarter k = 4 * (tile index of this CTA) + q

@@ -21,6 +21,11 @@ struct Geom {
     // links in K1, forward Delta~ in K5) is re-read from L2 one z-block later, not from DRAM one t-slice later.
     int zb;
     unsigned int zb_magic, nb3_magic;     // ceil(2^32 / zb), ceil(2^32 / nb3)  (0 when the divisor is 1)
+    // batched contexts (lgf_create_batch: B independent lattices of the same shape per launch): blockIdx.z =
+    // b * nzt + (z,t) tile, nzt = nb2 * nb3; every field of lattice b sits b * (its size) behind lattice 0's
+    int nzt;
+    unsigned int nzt_magic;
+    int nblocks;                          // CTAs per lattice = nb0 * nb1 * nzt (segment of the partials array)
 };
 
 // The site kernels are launched on a 3-D grid (x tiles, y tiles, z tiles * t tiles): same CTA order as a linear
@@ -34,6 +39,18 @@ __device__ __forceinline__ void split_zt(const Geom& g, unsigned bzt, unsigned& 
     bz = zblk * (unsigned)g.zb + zi;
 }
 __device__ __forceinline__ unsigned linear_block() { return blockIdx.x + gridDim.x * (blockIdx.y + gridDim.y * blockIdx.z); }
+// which lattice of the batch and which (z,t) tile inside it a grid z index means (z < 2^16: exact multiply-high quotient)
+struct BatchPos { unsigned b, bzt; };
+__device__ __forceinline__ BatchPos batch_pos(const Geom& g, unsigned z) {
+    BatchPos p;
+    p.b = div_magic(z, g.nzt_magic);
+    p.bzt = z - p.b * (unsigned)g.nzt;
+    return p;
+}
+// index of this CTA's (theta, F) partial: lattice b's segment, the CTA's position inside its lattice
+__device__ __forceinline__ unsigned partial_index(const Geom& g, const BatchPos& p) {
+    return p.b * (unsigned)g.nblocks + blockIdx.x + gridDim.x * (blockIdx.y + gridDim.y * p.bzt);
+}
 
 // Loop / reduction state, lives in the workspace (device memory).
 struct DevState {
@@ -66,12 +83,13 @@ struct SiteTile {
     // thread -> lattice coordinates of its site; returns false outside the lattice
     // REVERSE: walk the tiles from the last to the first.  K1 does (it follows K5, which walks forward, so the
     // links K5 wrote last are still in L2 when K1 starts with them).
+    // bp: batch_pos of blockIdx.z (REVERSE: of gridDim.z - 1 - blockIdx.z)
     template <bool REVERSE = false>
-    __device__ static __forceinline__ bool coords(const Geom& g, int x[4]) {
+    __device__ static __forceinline__ bool coords(const Geom& g, const BatchPos& bp, int x[4]) {
         const unsigned bx = REVERSE ? gridDim.x - 1 - blockIdx.x : blockIdx.x;
         const unsigned by = REVERSE ? gridDim.y - 1 - blockIdx.y : blockIdx.y;
         unsigned bz, bt;
-        split_zt(g, REVERSE ? gridDim.z - 1 - blockIdx.z : blockIdx.z, bz, bt);
+        split_zt(g, bp.bzt, bz, bt);
         int t = threadIdx.x;
         x[0] = bx * TX + t % TX; t /= TX;
         x[1] = by * TY + t % TY; t /= TY;
@@ -143,13 +161,21 @@ __global__ void __launch_bounds__(Tile::kThreads, SiteOcc<T, NC>::k1)
 k1_delta_theta_F(const Cx<T>* __restrict__ U, Cx<T>* __restrict__ D, double2* __restrict__ partials,
                  DevState* st, Geom g, int mode) {
     pdl_entry();
+#ifndef LGF_K1_FORWARD
+    const BatchPos bp = batch_pos(g, gridDim.z - 1 - blockIdx.z);
+#else
+    const BatchPos bp = batch_pos(g, blockIdx.z);
+#endif
+    st += bp.b;
+    U += (size_t)bp.b * 4 * NC * g.V;
+    D += (size_t)bp.b * 4 * g.V;
     if (mode == 1 && *reinterpret_cast<const volatile int*>(&st->done)) return;
-    if (mode == 1 && threadIdx.x == 0 && linear_block() == 0) st->pending = 1;    // folded in by the next k1_finish
+    if (mode == 1 && threadIdx.x == 0 && partial_index(g, bp) == bp.b * (unsigned)g.nblocks) st->pending = 1;    // folded in by the next k1_finish
     int x[4];
 #ifndef LGF_K1_FORWARD
-    const bool valid = Tile::template coords<true>(g, x);
+    const bool valid = Tile::template coords<true>(g, bp, x);
 #else
-    const bool valid = Tile::template coords<false>(g, x);
+    const bool valid = Tile::template coords<false>(g, bp, x);
 #endif
     double th = 0.0, fn = 0.0;
     if (valid) {
@@ -197,7 +223,7 @@ k1_delta_theta_F(const Cx<T>* __restrict__ U, Cx<T>* __restrict__ D, double2* __
         fn = (double)retr;
     }
     block_sum2<Tile::kThreads>(th, fn);
-    if (threadIdx.x == 0) partials[linear_block()] = make_double2(th, fn);   // summed by k1_finish
+    if (threadIdx.x == 0) partials[partial_index(g, bp)] = make_double2(th, fn);   // summed by k1_finish
 }
 
 // Second half of K1: one CTA sums the per-CTA (theta, F) partials in index order (deterministic, no
@@ -209,6 +235,8 @@ constexpr int kFinishThreads = 1024;
 __global__ void __launch_bounds__(kFinishThreads)
 k1_finish(const double2* __restrict__ partials, int n, DevState* st, double V, int mode) {
     pdl_entry();
+    partials += (size_t)blockIdx.x * n;          // one CTA per lattice of a batched context
+    st += blockIdx.x;
     if (mode >= 1 && *reinterpret_cast<volatile int*>(&st->done)) return;
     // mode 3: deferred end of an iteration -- launched beside the NEXT iteration's K2 (and once after the last
     // iteration of a batch); a no-op when the previous K1 has been folded in already
@@ -250,9 +278,13 @@ template <typename T, int NC, class Tile>
 __global__ void __launch_bounds__(Tile::kThreads, SiteOcc<T, NC>::k5)
 k5_gbuild_update(Cx<T>* __restrict__ U, const Cx<T>* __restrict__ D, const DevState* st, Geom g, T half_alpha) {
     pdl_entry();
+    const BatchPos bp = batch_pos(g, blockIdx.z);
+    st += bp.b;
+    U += (size_t)bp.b * 4 * NC * g.V;
+    D += (size_t)bp.b * 4 * g.V;
     if (*reinterpret_cast<const volatile int*>(&st->done)) return;
     int x[4];
-    if (!Tile::coords(g, x)) return;
+    if (!Tile::coords(g, bp, x)) return;
     const long long s = site_index(g, x);
     constexpr int NR = NC / 3;  // rows to produce: 3 or 2
     Su3<T> g0;

@@ -16,10 +16,10 @@ struct SiteTileMu {
     static constexpr int kThreads = 4 * kSites;
     static_assert(kSites % 32 == 0, "mu must be warp-uniform");
     static constexpr int tx = TX, ty = TY, tz = TZ, tt = TT;
-    __device__ static __forceinline__ bool coords(const Geom& g, int ls, int x[4]) {
+    __device__ static __forceinline__ bool coords(const Geom& g, const BatchPos& bp, int ls, int x[4]) {
         const unsigned bx = blockIdx.x, by = blockIdx.y;
         unsigned bz, bt;
-        split_zt(g, blockIdx.z, bz, bt);
+        split_zt(g, bp.bzt, bz, bt);
         x[0] = bx * TX + ls % TX; ls /= TX;
         x[1] = by * TY + ls % TY; ls /= TY;
         x[2] = bz * TZ + ls % TZ; ls /= TZ;
@@ -42,11 +42,15 @@ template <typename T, int NC, class Tile>
 __global__ void __launch_bounds__(Tile::kThreads, SiteOcc<T, NC>::k5m)
 k5m_gbuild_update(Cx<T>* __restrict__ U, const Cx<T>* __restrict__ D, const DevState* st, Geom g, T half_alpha) {
     pdl_entry();
+    const BatchPos bp = batch_pos(g, blockIdx.z);
+    st += bp.b;
+    U += (size_t)bp.b * 4 * NC * g.V;
+    D += (size_t)bp.b * 4 * g.V;
     if (*reinterpret_cast<const volatile int*>(&st->done)) return;
     constexpr int NS = Tile::kSites;
     const int ls = threadIdx.x % NS, mu = threadIdx.x / NS;
     int x[4];
-    if (!Tile::coords(g, ls, x)) return;
+    if (!Tile::coords(g, bp, ls, x)) return;
     const long long s = site_index(g, x);
     long long stride; int xm, Lm;
     dir_info(g, mu, x, stride, xm, Lm);
@@ -106,11 +110,15 @@ template <typename T, int NC, class Tile, int MINB>
 __global__ void __launch_bounds__(Tile::kThreads, MINB)
 k5s_gbuild_update(Cx<T>* __restrict__ U, const Cx<T>* __restrict__ D, const DevState* st, Geom g, T half_alpha) {
     pdl_entry();
+    const BatchPos bp = batch_pos(g, blockIdx.z);
+    st += bp.b;
+    U += (size_t)bp.b * 4 * NC * g.V;
+    D += (size_t)bp.b * 4 * g.V;
     if (*reinterpret_cast<const volatile int*>(&st->done)) return;
     constexpr int TX = Tile::tx, TY = Tile::ty, TZ = Tile::tz, TT = Tile::tt, NS = Tile::kSites, NG = Tile::NG, NR = NC / 3;
     __shared__ Cx<T> G[9 * NG];
     unsigned bz, bt;
-    split_zt(g, blockIdx.z, bz, bt);
+    split_zt(g, bp.bzt, bz, bt);
     const int x0 = blockIdx.x * TX, y0 = blockIdx.y * TY, z0 = bz * TZ, t0 = bt * TT;
     const int s1 = g.L[0], s2 = s1 * g.L[1], s3 = s2 * g.L[2];      // 32-bit site arithmetic (V < 2^31)
     const int tid = threadIdx.x, ls = tid % NS, mu = tid / NS;

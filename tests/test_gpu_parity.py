@@ -557,3 +557,57 @@ def test_wilson_lines_and_singlet_correlator(L):
         Co32 = oracle.singlet_correlator(L, gi.from_real(U32))
         assert np.max(np.abs(torch.view_as_complex(gf.singlet_correlator().to(torch.float64)).numpy() - Co32)) <= 2e-5
     gf.close()
+
+
+@pytest.mark.parametrize("L,nbatch", [((8, 8, 8, 8), 5), ((16, 16, 16, 16), 3), ((6, 4, 12, 8), 2), ((16, 16, 8, 8), 4)])
+@pytest.mark.parametrize("prec,stor", MODES)
+def test_batched_context_equals_single_lattice_contexts(L, nbatch, prec, stor):
+    """lgf_create_batch: nbatch different lattices fixed by the same launches.  Each lattice must
+    come out exactly as from a context of its own (same kernels, same per-lattice reduction order: bitwise), with its
+    own iteration count -- the lattices converge at different iterations -- and lattice 0 must match the oracle."""
+    Us = [gi.make_config(L, 80 + b, 0.59 if b % 2 == 0 else 0.57) for b in range(nbatch)]
+    stack = torch.cat([gi.as_real(u) for u in Us], 0)
+    gb = lgf.GaugeFixer(L, prec, stor, nbatch=nbatch)
+    gb.load(stack)
+    m = gb.measure()
+    rb = gb.iterate(2, ALPHA)
+    after2 = gb.store().reshape(nbatch, -1, 4, 3, 3, 2)
+    gb.load(stack.cuda())
+    rf = gb.fix(ALPHA, 1e-10, 500)
+    fixed = gb.store(device="cuda").cpu().reshape(nbatch, -1, 4, 3, 3, 2)
+    assert len({r.iterations for r in rf}) > 1 or nbatch < 3          # the crossings differ between the lattices
+    for b in range(nbatch):
+        g1 = _fixer(L, prec, stor, Us[b])
+        m1 = g1.measure()
+        assert (m[b].theta, m[b].F) == (m1.theta, m1.F)
+        r1 = g1.iterate(2, ALPHA)
+        assert (rb[b].theta, rb[b].F, rb[b].iterations) == (r1.theta, r1.F, 2)
+        assert torch.equal(after2[b], g1.store())
+        g1.load(gi.as_real(Us[b]))
+        f1 = g1.fix(ALPHA, 1e-10, 500)
+        assert (rf[b].iterations, rf[b].theta, rf[b].F, rf[b].converged) == (f1.iterations, f1.theta, f1.F, True)
+        assert torch.equal(fixed[b], g1.store())
+        g1.close()
+    ref, n, theta, F, _, _ = oracle.fix(L, Us[0], ALPHA, 1e-10, 500)
+    assert rf[0].iterations == n and abs(rf[0].theta - theta) <= 1e-10 * theta and abs(rf[0].F - F) <= 1e-10 * F
+    assert np.max(np.abs(_cplx(fixed[0]) - ref)) <= 1e-11
+    r3 = gb.iterate(3, ALPHA)                                          # a batched fix leaves Delta stale: iterate re-measures
+    assert all(r.iterations == 3 for r in r3) and all(r.theta < 1e-10 for r in r3)
+    gb.close()
+
+
+def test_batched_context_fp32_and_limits():
+    L = (8, 8, 8, 8)
+    Us = [gi.as_real(gi.make_config(L, 90 + b, 0.59), torch.float32) for b in range(4)]
+    gb = lgf.GaugeFixer(L, lgf.LGF_F32, lgf.LGF_REAL12, nbatch=4)
+    gb.load(torch.cat(Us, 0))
+    rb = gb.iterate(3, ALPHA)
+    out = gb.store().reshape(4, -1, 4, 3, 3, 2)
+    for b in range(4):
+        ref, thh, Fh = oracle.iterate(L, gi.from_real(Us[b]), 3, ALPHA)
+        assert np.max(np.abs(_cplx(out[b]) - ref)) <= 2e-5 and abs(rb[b].F - Fh[3]) <= 1e-5 * abs(Fh[3])
+    with pytest.raises(lgf.LgfError):
+        gb.singlet_correlator()                                         # single-lattice contexts only
+    gb.close()
+    assert lgf.workspace_bytes(L, lgf.LGF_F32, lgf.LGF_REAL12, nbatch=4) > 3.9 * lgf.workspace_bytes(L, lgf.LGF_F32, lgf.LGF_REAL12) - (1 << 22)
+    assert lgf.workspace_bytes(L, lgf.LGF_F32, lgf.LGF_REAL12, nbatch=5000) == 0      # grid z = nbatch x (z,t) tiles < 2^16
