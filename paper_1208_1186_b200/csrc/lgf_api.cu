@@ -42,8 +42,8 @@ int cuda_fail(cudaError_t e, const char* what) {
 // Developer A/B knobs (LGF_ZBLOCK, LGF_SITE_TILE, LGF_FUSED, ...; DESIGN.md §6 "A/B knobs") are read only when
 // LGF_DEVKNOBS=1 is set: a production process cannot change which kernels run through a stray environment variable.
 const char* knob(const char* name) {
-    static const bool enabled = [] { const char* e = getenv("LGF_DEVKNOBS"); return e && atoi(e) != 0; }();
-    return enabled ? getenv(name) : nullptr;
+    const char* on = getenv("LGF_DEVKNOBS");          // read at every lgf_create (tests switch it per case)
+    return (on && atoi(on) != 0) ? getenv(name) : nullptr;
 }
 bool fused_requested() { const char* e = knob("LGF_FUSED"); return e && atoi(e) != 0; }
 
