@@ -2,6 +2,10 @@
  * lgf_create_simple, lgf_load / lgf_store with HOST buffers, lgf_measure, lgf_iterate, lgf_fix, error codes.
  * Expected values are closed forms (SURVEY.md §8(c) pins P3, P6): for an x-independent field U_mu(x) = V_mu
  * Delta = 0, so theta = 0 and F = (1/12) sum_mu Re Tr V_mu, and the field is a fixed point of the iteration.
+ * On the same field the temporal Wilson line is V_t^Lt at every site, so the singlet correlator (eq. (1))
+ * is 1 for every r.  lgf_create_batch needs a caller-allocated DEVICE workspace, which this CUDA-free program cannot
+ * make: the batch entry points are exercised through lgf_batch_size and lgf_workspace_bytes_batch only (the batched
+ * iteration itself: tests/test_gpu_parity.py).
  * Built and run by tests/test_c_abi.py; exit code 0 = all checks passed. */
 #include <math.h>
 #include <stdio.h>
@@ -83,6 +87,39 @@ static int run(int precision, int storage) {
         for (size_t i = 0; i < (size_t)V * 72; ++i) md = fmax(md, fabs((double)o[i] - (double)hf[i]));
         CHECK(md <= 2e-6);
         free(o);
+    }
+    /* the step after the path: W(x) = V_t^Lt = diag(e^{i Lt a_t}, e^{i Lt b_t}, e^{-i Lt (a_t+b_t)}), C(r) = 1 */
+    {
+        const long long Vs = V / L[3];
+        const double wtol = precision == LGF_F64 ? 1e-12 : 2e-5;
+        const double ph[3] = {L[3] * a[3], L[3] * b[3], -L[3] * (a[3] + b[3])};
+        if (precision == LGF_F64) {
+            double* w = (double*)malloc(sizeof(double) * (size_t)Vs * 18);
+            double* cr = (double*)malloc(sizeof(double) * (size_t)Vs * 2);
+            CHECK(w && cr && lgf_wilson_lines(ctx, w, LGF_HOST) == LGF_OK && lgf_singlet_correlator(ctx, cr, LGF_HOST) == LGF_OK);
+            double md = 0.0;
+            for (long long x = 0; x < Vs; ++x)
+                for (int i = 0; i < 3; ++i)
+                    for (int j = 0; j < 3; ++j) {
+                        const double re = i == j ? cos(ph[i]) : 0.0, im = i == j ? sin(ph[i]) : 0.0;
+                        md = fmax(md, fmax(fabs(w[(x * 9 + 3 * i + j) * 2] - re), fabs(w[(x * 9 + 3 * i + j) * 2 + 1] - im)));
+                    }
+            for (long long x = 0; x < Vs; ++x) md = fmax(md, fmax(fabs(cr[2 * x] - 1.0), fabs(cr[2 * x + 1])));
+            CHECK(md <= wtol);
+            free(w);
+            free(cr);
+        } else {
+            float* cr = (float*)malloc(sizeof(float) * (size_t)Vs * 2);
+            CHECK(cr && lgf_singlet_correlator(ctx, cr, LGF_HOST) == LGF_OK);
+            double md = 0.0;
+            for (long long x = 0; x < Vs; ++x) md = fmax(md, fmax(fabs((double)cr[2 * x] - 1.0), fabs((double)cr[2 * x + 1])));
+            CHECK(md <= wtol);
+            free(cr);
+        }
+        CHECK(lgf_iterate(ctx, 1, 0.08, &r) == LGF_OK && r.iterations == 1 && fabs(r.F - Fexp) <= tol);   /* scratch use is harmless */
+        CHECK(lgf_batch_size(ctx) == 1);
+        CHECK(lgf_workspace_bytes_batch(L, precision, storage, 3) > 2 * lgf_workspace_bytes(L, precision, storage));
+        CHECK(lgf_workspace_bytes_batch(L, precision, storage, 0) == 0);
     }
     /* argument errors leave *out untouched */
     r.iterations = -7;
