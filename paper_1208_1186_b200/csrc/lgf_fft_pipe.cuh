@@ -68,9 +68,72 @@ template <typename T, int NX> struct XySwz {
     static constexpr int mask = (NX < kSlots ? NX : kSlots) - 1;
 };
 
+// v[k] *= exp(SIGN 2 pi i r k / N) for k = 1..NK-1; r in [0, NR) is a run-time value that is uniform across the warp at
+// every call site (the branches below do not diverge); the factors are compile-time literals.
+template <int N, int NK, int NR, int SIGN, typename T>
+__device__ __forceinline__ void tw_rows(Cx<T>* v, int r) {
+    static_for<1, NR>([&](auto rr) {
+        if (r == rr.value) static_for<1, NK>([&](auto k) { v[k.value] = mul_tw<rr.value * k.value, N, SIGN, T>(v[k.value]); });
+    });
+}
+
+// K2 in THREE register stages per plane instead of four (the structure of lgf_fft_pipe3.cuh's K3, here for the (x,y)
+// plane): with y lines split N_y = A*B (A first, 12 or 16) and x lines N_x = C*D (C = 4 first, D = 12 or 16)
+//   P1  thread (x, n2y):    DFT_A over m of rows n2y + B m, times w_Ny^{-n2y k1y}        (lanes along x; dense in, swizzled out)
+//   P2  thread (n2x, k1y):  DFT_B over the rows k1y*B + j, then DFT_C over the columns n2x + D m   (a B x C block; lanes along x)
+//   P3  thread (y, k1x):    times w_Nx^{-j k1x}, DFT_D over the columns k1x*D + j         (lanes along y)
+// The spectrum is left in the digit-swapped order of LineSplit<Ny, A> / LineSplit<Nx, C>; K4 inverts it with its
+// two-stage passes on the same splits.  P1's output columns are another lane's input columns: a warp-level barrier
+// separates its loads from its stores (the swizzle permutes inside aligned 8- or 16-element groups: inside a warp).
+template <typename T, class SX, class SY, int PB, int GT, int NG>
+__device__ __forceinline__ void xy3_forward_passes(Cx<T>* tile, int g, int gtid) {
+    constexpr int NX = SX::kN, NY = SY::kN, PLANE = NX * NY, SW = XySwz<T, NX>::mask;
+    constexpr int A = SY::kN1, B = SY::kN2, C = SX::kN1, D = SX::kN2;
+    static_assert(B > 1 && D > 1 && B * C <= 16, "three-stage K2: the middle block must fit the registers");
+    static_assert((PB * NX * B) % 32 == 0, "P1 must fill whole warps (its lanes exchange positions)");
+    for (int it = gtid; it < PB * NX * B; it += GT) {
+        const int x = it % NX, n2 = (it / NX) % B, pl = it / (NX * B);
+        Cx<T>* s = tile + pl * PLANE;
+        Cx<T> v[A];
+        static_for<0, A>([&](auto m) { v[m.value] = s[(n2 + B * m.value) * NX + x]; });
+        __syncwarp();
+        RegFft<A, -1, T>::run(v);
+        tw_rows<NY, A, B, -1, T>(v, n2);
+        static_for<0, A>([&](auto k1) { constexpr int r0 = k1.value * B; const int r = r0 + n2; s[r * NX + (x ^ (r & SW))] = v[k1.value]; });
+    }
+    named_bar_sync(1 + g, GT);
+    for (int it = gtid; it < PB * D * A; it += GT) {
+        const int n2x = it % D, k1y = (it / D) % A, pl = it / (D * A);
+        Cx<T>* s = tile + pl * PLANE + k1y * B * NX;
+        Cx<T> e[C][B];
+        static_for<0, C>([&](auto m) {
+            static_for<0, B>([&](auto j) { e[m.value][j.value] = s[j.value * NX + ((n2x + D * m.value) ^ ((k1y * B + j.value) & SW))]; });
+            RegFft<B, -1, T>::run(e[m.value]);
+        });
+        static_for<0, B>([&](auto j) {
+            Cx<T> u[C];
+            static_for<0, C>([&](auto m) { u[m.value] = e[m.value][j.value]; });
+            RegFft<C, -1, T>::run(u);
+            static_for<0, C>([&](auto k1x) { s[j.value * NX + ((k1x.value * D + n2x) ^ ((k1y * B + j.value) & SW))] = u[k1x.value]; });
+        });
+    }
+    named_bar_sync(1 + g, GT);
+    for (int it = gtid; it < PB * NY * C; it += GT) {
+        const int y = it % NY, k1x = (it / NY) % C, pl = it / (NY * C);
+        Cx<T>* s = tile + pl * PLANE + y * NX;
+        const int sw = y & SW;
+        Cx<T> v[D];
+        static_for<0, D>([&](auto j) { v[j.value] = s[(k1x * D + j.value) ^ sw]; });
+        tw_rows<NX, D, C, -1, T>(v, k1x);
+        RegFft<D, -1, T>::run(v);
+        static_for<0, D>([&](auto j) { s[(k1x * D + j.value) ^ sw] = v[j.value]; });
+    }
+    named_bar_sync(1 + g, GT);
+}
+
 // K2 (SIGN = -1: natural in -> layout B out) / K4 (SIGN = +1: natural in -> natural out, in place
 // allowed); tile = PB contiguous (x,y) planes.
-template <typename T, class SX, class SY, int SIGN, int PB, int GT, int NG, int NBUF>
+template <typename T, class SX, class SY, int SIGN, int PB, int GT, int NG, int NBUF, bool THREE = false>
 __global__ void __launch_bounds__(GT * NG, 1)
 fft_xy_pipe(const Cx<T>* in, Cx<T>* out, const XyPipeArgs A, const int* done) {
     pdl_entry();
@@ -113,7 +176,9 @@ fft_xy_pipe(const Cx<T>* in, Cx<T>* out, const XyPipeArgs A, const int* done) {
         mbar_wait(&full[buf], (uint32_t)((i / NBUF) & 1));
         // (planes past nvalid hold stale data: they are transformed like the others, never stored)
 
-        if (SIGN < 0) {
+        if constexpr (SIGN < 0 && THREE) {
+            xy3_forward_passes<T, SX, SY, PB, GT, NG>(tile, g, gtid);
+        } else if (SIGN < 0) {
             // ---- y axis: A (threads along x; dense in, swizzled out), B ----
             for (int it = gtid; it < PB * NX * SY::kN2; it += GT) {
                 const int x = it % NX, n2 = (it / NX) % SY::kN2, pl = it / (NX * SY::kN2);
@@ -159,21 +224,23 @@ fft_xy_pipe(const Cx<T>* in, Cx<T>* out, const XyPipeArgs A, const int* done) {
         }
         // ---- x axis (threads along y; every position swizzled by the row's low bits) ----
         if (SIGN < 0) {
-            for (int it = gtid; it < PB * NY * SX::kN2; it += GT) {
-                const int y = it % NY, n2 = (it / NY) % SX::kN2, pl = it / (NY * SX::kN2);
-                Cx<T>* s = tile + pl * PLANE + y * NX;
-                const int sw = y & SW;
-                stage_A_fwd<T, SX>(n2, twx, [&](int p) { return s[p ^ sw]; }, [&](int p, Cx<T> v) { s[p ^ sw] = v; });
-            }
-            group_sync<GT, NG>(g);
-            if constexpr (SX::kN2 > 1) {
-                for (int it = gtid; it < PB * NY * SX::kN1; it += GT) {
-                    const int y = it % NY, k1 = (it / NY) % SX::kN1, pl = it / (NY * SX::kN1);
+            if constexpr (!THREE) {
+                for (int it = gtid; it < PB * NY * SX::kN2; it += GT) {
+                    const int y = it % NY, n2 = (it / NY) % SX::kN2, pl = it / (NY * SX::kN2);
                     Cx<T>* s = tile + pl * PLANE + y * NX;
                     const int sw = y & SW;
-                    stage_B<T, SX, 1, 0>(k1, twx, [&](int p) { return s[p ^ sw]; }, [&](int p, Cx<T> v) { s[p ^ sw] = v; }, NoScale());
+                    stage_A_fwd<T, SX>(n2, twx, [&](int p) { return s[p ^ sw]; }, [&](int p, Cx<T> v) { s[p ^ sw] = v; });
                 }
                 group_sync<GT, NG>(g);
+                if constexpr (SX::kN2 > 1) {
+                    for (int it = gtid; it < PB * NY * SX::kN1; it += GT) {
+                        const int y = it % NY, k1 = (it / NY) % SX::kN1, pl = it / (NY * SX::kN1);
+                        Cx<T>* s = tile + pl * PLANE + y * NX;
+                        const int sw = y & SW;
+                        stage_B<T, SX, 1, 0>(k1, twx, [&](int p) { return s[p ^ sw]; }, [&](int p, Cx<T> v) { s[p ^ sw] = v; }, NoScale());
+                    }
+                    group_sync<GT, NG>(g);
+                }
             }
             // ---- scatter CXB-site chunks into layout B (its tiles are stored padded, as K3 wants them in smem) ----
             const int cxb_mask = (1 << A.cxb_shift) - 1;

@@ -28,15 +28,6 @@
 
 namespace lgf {
 
-// v[k] *= exp(SIGN 2 pi i r k / N) for k = 1..NK-1; r in [0, NR) is a run-time value that is uniform across the warp at
-// every call site (the branches below do not diverge); the factors are compile-time literals.
-template <int N, int NK, int NR, int SIGN, typename T>
-__device__ __forceinline__ void tw_rows(Cx<T>* v, int r) {
-    static_for<1, NR>([&](auto rr) {
-        if (r == rr.value) static_for<1, NK>([&](auto k) { v[k.value] = mul_tw<rr.value * k.value, N, SIGN, T>(v[k.value]); });
-    });
-}
-
 // Pass bodies.  ROW(t) -> pointer to element (z position 0, cx 0) of row t of the tile in shared memory; element
 // (zp, cx) of that row sits at [zp * CX + cx].  `it` enumerates a pass's work items, cx fastest.
 template <typename T, class SZ, class ST_, int CX>

@@ -21,6 +21,32 @@ struct XyP {
     }
 };
 
+// K2 in three register stages per plane (xy3_forward_passes); K4 on the same line splits in two stages
+template <typename T, int NX, int X1, int NY, int Y1, int PB, int GT, int NG, int NBUF>
+struct XyP3 {
+    typedef LineSplit<NX, X1> SX;
+    typedef LineSplit<NY, Y1> SY;
+    static constexpr size_t kSmem = sizeof(Cx<T>) * (size_t)NBUF * PB * NX * NY + 8 * NBUF;
+    static_assert(kSmem <= 227 * 1024, "tile ring exceeds shared memory");
+    static XyPipeEntry entry() {
+        return XyPipeEntry{NX, NY, X1, Y1, PB, GT * NG, NBUF, kSmem,
+                           (const void*)&fft_xy_pipe<T, SX, SY, -1, PB, GT, NG, NBUF, true>,
+                           (const void*)&fft_xy_pipe<T, SX, SY, +1, PB, GT, NG, NBUF, false>, 0};
+    }
+};
+// ... and through the I/O warp
+template <typename T, int NX, int X1, int NY, int Y1, int PB, int GT, int NG, int NBUF>
+struct XyPIO3 {
+    typedef LineSplit<NX, X1> SX;
+    typedef LineSplit<NY, Y1> SY;
+    static constexpr size_t kSmem = sizeof(Cx<T>) * (size_t)NBUF * PB * NX * NY + 16 * NBUF;
+    static_assert(kSmem <= 227 * 1024, "tile ring exceeds shared memory");
+    static XyPipeEntry entry() {
+        return XyPipeEntry{NX, NY, X1, Y1, PB, GT * NG + 32, NBUF, kSmem,
+                           (const void*)&fft_xy_pipe_io<T, SX, SY, -1, PB, GT, NG, NBUF, true>, nullptr, 1};
+    }
+};
+
 // K2 through the I/O warp and TMA tensor stores (fft_xy_pipe_io); K4 of such a lattice runs on a plain XyP entry
 template <typename T, int NX, int X1, int NY, int Y1, int PB, int GT, int NG, int NBUF>
 struct XyPIO {

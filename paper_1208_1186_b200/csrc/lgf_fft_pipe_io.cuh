@@ -52,7 +52,7 @@ __device__ __forceinline__ void io_lane_loop(int my_tiles, uint64_t* done, FETCH
 // K2 (SIGN = -1: natural in -> layout B out) / K4 (SIGN = +1: natural in -> natural out, in place
 // allowed); tile = PB contiguous (x,y) planes.
 // `bmap`: CUtensorMap of layout B as the 4-D tensor (2 reals x CXB sites, z, t row, tile) -- used by K2 only.
-template <typename T, class SX, class SY, int SIGN, int PB, int GT, int NG, int NBUF>
+template <typename T, class SX, class SY, int SIGN, int PB, int GT, int NG, int NBUF, bool THREE = false>
 __global__ void __launch_bounds__(GT * NG + 32, 1)
 fft_xy_pipe_io(const Cx<T>* in, Cx<T>* out, const __grid_constant__ XyPipeArgs A, const int* done_flag,
             const __grid_constant__ CUtensorMap bmap) {
@@ -119,7 +119,9 @@ fft_xy_pipe_io(const Cx<T>* in, Cx<T>* out, const __grid_constant__ XyPipeArgs A
         mbar_wait(&full[buf], (uint32_t)((i / NBUF) & 1));
         // (planes past the last valid one hold stale data: they are transformed like the others, never stored)
 
-        if (SIGN < 0) {
+        if constexpr (SIGN < 0 && THREE) {
+            xy3_forward_passes<T, SX, SY, PB, GT, NG>(tile, g, gtid);
+        } else if (SIGN < 0) {
             // ---- y axis: A (threads along x; dense in, swizzled out), B ----
             for (int it = gtid; it < PB * NX * SY::kN2; it += GT) {
                 const int x = it % NX, n2 = (it / NX) % SY::kN2, pl = it / (NX * SY::kN2);
@@ -165,21 +167,23 @@ fft_xy_pipe_io(const Cx<T>* in, Cx<T>* out, const __grid_constant__ XyPipeArgs A
         }
         // ---- x axis (threads along y; every position swizzled by the row's low bits) ----
         if (SIGN < 0) {
-            for (int it = gtid; it < PB * NY * SX::kN2; it += GT) {
-                const int y = it % NY, n2 = (it / NY) % SX::kN2, pl = it / (NY * SX::kN2);
-                Cx<T>* s = tile + pl * PLANE + y * NX;
-                const int sw = y & SW;
-                stage_A_fwd<T, SX>(n2, twx, [&](int p) { return s[p ^ sw]; }, [&](int p, Cx<T> v) { s[p ^ sw] = v; });
-            }
-            named_bar_sync(1 + g, GT);
-            if constexpr (SX::kN2 > 1) {
-                for (int it = gtid; it < PB * NY * SX::kN1; it += GT) {
-                    const int y = it % NY, k1 = (it / NY) % SX::kN1, pl = it / (NY * SX::kN1);
+            if constexpr (!THREE) {
+                for (int it = gtid; it < PB * NY * SX::kN2; it += GT) {
+                    const int y = it % NY, n2 = (it / NY) % SX::kN2, pl = it / (NY * SX::kN2);
                     Cx<T>* s = tile + pl * PLANE + y * NX;
                     const int sw = y & SW;
-                    stage_B<T, SX, 1, 0>(k1, twx, [&](int p) { return s[p ^ sw]; }, [&](int p, Cx<T> v) { s[p ^ sw] = v; }, NoScale());
+                    stage_A_fwd<T, SX>(n2, twx, [&](int p) { return s[p ^ sw]; }, [&](int p, Cx<T> v) { s[p ^ sw] = v; });
                 }
                 named_bar_sync(1 + g, GT);
+                if constexpr (SX::kN2 > 1) {
+                    for (int it = gtid; it < PB * NY * SX::kN1; it += GT) {
+                        const int y = it % NY, k1 = (it / NY) % SX::kN1, pl = it / (NY * SX::kN1);
+                        Cx<T>* s = tile + pl * PLANE + y * NX;
+                        const int sw = y & SW;
+                        stage_B<T, SX, 1, 0>(k1, twx, [&](int p) { return s[p ^ sw]; }, [&](int p, Cx<T> v) { s[p ^ sw] = v; }, NoScale());
+                    }
+                    named_bar_sync(1 + g, GT);
+                }
             }
         } else {
             if constexpr (SX::kN2 > 1) {
