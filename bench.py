@@ -172,6 +172,18 @@ def workload_name(L, prec: str, stor: int, plaq_target: float) -> str:
             f"+ Haar gauge transform, alpha {ALPHA}")
 
 
+def config_dict(L, prec: str, stor: int, plaq_target: float, plaq: float, world: int, peak: float, peak_src: str) -> dict:
+    """`config` of the JSON line -- the SAME dictionary in the CUDA arm and in the reference arm (the oracle computes in
+    fp64 on full 3x3 links whatever `prec` / `stor` say: they name the workload the ratio is taken on)."""
+    V = L[0] * L[1] * L[2] * L[3]
+    w = 8 if prec == "f64" else 4
+    return {"workload": workload_name(L, prec, stor, plaq_target), "measured_plaquette": round(plaq, 6), "sites": V,
+            "parallelism": "replicas only" if world > 1 else "1 GPU",
+            "l2": ("inputs larger than L2 (links %.0f MB > 126 MB)" if 4 * stor * V * w > 126e6 else
+                   "L2-resident workload (links %.0f MB): launch-bound, reported without a roofline claim") % (4 * stor * V * w / 1e6),
+            "hbm_peak_GBps": peak, "hbm_peak_source": peak_src}
+
+
 def run_reference(args, L):
     """--impl reference: the oracle (unmodified, as it stands) on the box's host cores, same config / metric / unit as
     the CUDA arm; each step = one full oracle iteration of the same lattice (about 1 s at 32^4 on 16 threads), W warm-up
@@ -183,8 +195,11 @@ def run_reference(args, L):
     import lgf_inputs as gi
     V = gi.volume(L)
     dev = "cuda" if torch.cuda.is_available() else "cpu"
-    U = gi.make_config(L, gi.CONFIG_SEED + 2, args.plaquette, device=dev).cpu()
+    U = gi.make_config(L, gi.CONFIG_SEED + 2, args.plaquette, device=dev)
+    plaq = gi.mean_plaquette(U, L)
+    U = U.cpu()
     Ur = gi.as_real(U)
+    peak, peak_src = measured_peak()
     per_iter_cap = 60 if V <= (1 << 20) else 4
     steps = max(1, min(args.steps, per_iter_cap))
     warm = max(0, min(args.warmup, per_iter_cap - steps, 5))
@@ -197,8 +212,8 @@ def run_reference(args, L):
         "impl": "reference", "metric": "gauge_fix_iterations_per_s", "value": val, "unit": "iterations/s",
         "n_gpus": args.gpus, "steps": steps, "warmup": warm, "ms_per_step": 1e3 * sec / steps,
         "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
-        "config": {"workload": workload_name(L, args.precision, args.storage, args.plaquette), "sites": V,
-                   "note": "oracle/lgf_oracle.cpp (plain C++, fp64, full 3x3 links, OpenMP over sites/lines) on host cores"},
+        "config": config_dict(L, args.precision, args.storage, args.plaquette, plaq, 1, peak, peak_src),
+        "note": "oracle/lgf_oracle.cpp (plain C++, fp64, full 3x3 links, OpenMP over sites/lines) on host cores",
         "cpu_baseline": {"value": val, "unit": "iterations/s", "cores": thr, "kind": "oracle",
                          "sample": f"{steps} full iterations of the {lattice_name(L)} lattice"},
         "e2e": {"value": val, "unit": "iterations/s", "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
@@ -409,11 +424,7 @@ def main():
             "n_gpus": world, "steps": K, "warmup": W, "ms_per_step": pr["ms_per_iteration"],
             "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
             "dtype": primary[0], "data": "synthetic",
-            "config": {"workload": workload_name(L, primary[0], primary[1], args.plaquette),
-                       "measured_plaquette": plaq,
-                       "sites": V, "parallelism": "replicas only" if world > 1 else "1 GPU",
-                       "l2": "inputs larger than L2 (links %.0f MB > 126 MB)" % (4 * primary[1] * V * w / 1e6),
-                       "hbm_peak_GBps": peak, "hbm_peak_source": peak_src},
+            "config": config_dict(L, primary[0], primary[1], args.plaquette, plaq, world, peak, peak_src),
             "site_updates_per_s": pr["site_updates_per_s"],
             "achieved_HBM_GBps_algorithmic": pr["algorithmic_GBps"],
             "iteration_frac_of_hbm_roofline": pr["frac_of_hbm_peak"],

@@ -158,6 +158,11 @@ int lgf_profile_iterate(lgf_ctx* ctx, int64_t n, double alpha, double ms[5], lgf
  * info[2] = CTAs of the site kernel, info[3] = kernel launches per iteration (0 before the first run). */
 int lgf_path_info(const lgf_ctx* ctx, int32_t info[4]);
 
+/* Human-readable description of the kernels this context runs (which FFT path the lattice fell onto, line splits, tile
+ * shapes, K5 flavour), NUL-terminated into buf[0..n): a lattice whose extents are not instantiated (e.g. a 32 x 16
+ * (x,y) plane) runs on the slower one-tile-per-CTA or runtime-radix kernels, and this is where it says so. */
+int lgf_describe(const lgf_ctx* ctx, char* buf, size_t n);
+
 /* Number of kernel launches this context has enqueued since creation (for bench.py's gpu_launches). */
 int64_t lgf_launch_count(const lgf_ctx* ctx);
 

@@ -1,8 +1,13 @@
 """Seeded synthetic SU(3) lattice inputs (shared by the oracle tests, the GPU tests and bench.py).
 
 This module is the ONLY code that both sides of the parity check see.  It holds no step of the
-gauge-fixing method (no Delta, no FFT, no p^2 table, no reunitarised g-build); it only makes the
-*inputs* named by BASELINE.json `configs` (SURVEY.md §8(d) "Inputs"):
+gauge-fixing ITERATION (no Delta, no FFT, no p^2 table, no g-build from Delta~); it only makes the
+*inputs* named by BASELINE.json `configs` (SURVEY.md §8(d) "Inputs").  Two of its tools do restate
+formulas the method also uses, for the generator's own purposes: `su3_project` is a row Gram-Schmidt
+(SURVEY.md §8(c) reading #9's formula, used here to MAKE SU(3) matrices) and `gauge_transform` is
+U_mu(x) <- g(x) U_mu(x) g(x+mu)^dagger (step 5's formula, used here to scramble the gauge).  Neither the
+oracle nor the CUDA path calls them; tests use the second as an independent pin of the update's
+orientation.  The inputs:
 
 * rough links  U = SU3-projection of exp(i eps H),  H = sum_a xi_a lambda_a / 2,  xi_a ~ N(0,1),
   eps chosen so the mean plaquette hits a target (0.55 - 0.60, "beta ~ 6.0-like roughness");

@@ -80,6 +80,7 @@ def load_library() -> ctypes.CDLL:
     lib.lgf_singlet_correlator.argtypes = [vp, vp, ctypes.c_int]
     lib.lgf_debug_fourier_accelerate.argtypes = [vp]
     lib.lgf_path_info.argtypes = [vp, i32p]
+    lib.lgf_describe.argtypes = [vp, ctypes.c_char_p, ctypes.c_size_t]
     lib.lgf_launch_count.restype = ctypes.c_int64
     lib.lgf_launch_count.argtypes = [vp]
     for f in (lib.lgf_strerror, lib.lgf_last_error, lib.lgf_version):
@@ -209,6 +210,11 @@ class GaugeFixer:
         _check(self.lib.lgf_path_info(self._h, info), "lgf_path_info")
         return {"fft_path": ("runtime-radix", "compile-time", "pipelined")[info[0]], "fused": bool(info[1]),
                 "site_ctas": int(info[2]), "launches_per_iteration": int(info[3])}
+
+    def describe(self) -> str:
+        buf = ctypes.create_string_buffer(1024)
+        _check(self.lib.lgf_describe(self._h, buf, 1024), "lgf_describe")
+        return buf.value.decode()
 
     def profile_iterate(self, n: int, alpha: float):
         """-> (dict kernel name -> average ms per launch, LgfResult).  With the fused update kernel the

@@ -522,7 +522,10 @@ struct Impl {
 #define LGF_K1_CASE(ID, TILE) case ID: launch_ex(c, k1_delta_theta_F<T, NC, TILE>, grid3(c->geom, c->nbatch), dim3(TILE::kThreads), 0, \
             links(c), delta_src(c), partials, dev_state(c), c->geom, mode); break;
         switch (c->site_tile) {
-            LGF_K1_CASE(1, Tile1) LGF_K1_CASE(2, Tile2) LGF_K1_CASE(3, Tile3) LGF_K1_CASE(4, Tile4) LGF_K1_CASE(5, Tile5)
+            LGF_K1_CASE(1, Tile1) LGF_K1_CASE(4, Tile4)
+#ifdef LGF_DEV_VARIANTS
+            LGF_K1_CASE(2, Tile2) LGF_K1_CASE(3, Tile3) LGF_K1_CASE(5, Tile5)
+#endif
             default: launch_ex(c, k1_delta_theta_F<T, NC, Tile0>, grid3(c->geom, c->nbatch), dim3(Tile0::kThreads), 0,
                 links(c), delta_src(c), partials, dev_state(c), c->geom, mode);
         }
@@ -568,14 +571,20 @@ struct Impl {
             fused_entry<MarchTile<48, 4, 1>, 2>(),
             fused_entry<MarchTile<16, 4, 4>, 2>(),
             fused_entry<MarchTile<8, 8, 4>, 2>(),
+#ifdef LGF_DEV_VARIANTS      // measured and rejected: not in the default build
             fused_entry<MarchTile<32, 4, 4>, 1>(),
             fused_entry<MarchTile<48, 4, 2>, 1>(),
             fused_entry<MarchTile<64, 4, 2>, 1>(),
             fused_entry<MarchTile<32, 4, 2, true>, 1>(),
+#endif
         };
         return tab;
     }
+#ifdef LGF_DEV_VARIANTS
     static constexpr int kNumFused = 9;
+#else
+    static constexpr int kNumFused = 5;
+#endif
     // pick the marching tile for this lattice (LGF_FUSED = 0 disables the fused path, LGF_FUSED_TILE = i forces entry i)
     static int plan_fused(lgf_ctx* c) {
         c->fused_tile = -1;
@@ -645,7 +654,10 @@ struct Impl {
 #define LGF_K5_CASE(ID, TILE) case ID: launch_ex(c, k5_gbuild_update<T, NC, TILE>, grid3(c->geom, c->nbatch), dim3(TILE::kThreads), 0,  \
             links(c), delta(c), dev_state(c), c->geom, (T)(0.5 * alpha)); break;
         switch (c->site_tile) {
-            LGF_K5_CASE(1, Tile1) LGF_K5_CASE(2, Tile2) LGF_K5_CASE(3, Tile3) LGF_K5_CASE(4, Tile4) LGF_K5_CASE(5, Tile5)
+            LGF_K5_CASE(1, Tile1) LGF_K5_CASE(4, Tile4)
+#ifdef LGF_DEV_VARIANTS
+            LGF_K5_CASE(2, Tile2) LGF_K5_CASE(3, Tile3) LGF_K5_CASE(5, Tile5)
+#endif
             default: launch_ex(c, k5_gbuild_update<T, NC, Tile0>, grid3(c->geom, c->nbatch), dim3(Tile0::kThreads), 0, 
                 links(c), delta(c), dev_state(c), c->geom, (T)(0.5 * alpha));
         }
@@ -992,7 +1004,11 @@ static int create_common(const int32_t L[4], int precision, int storage, int nba
     {   // thread-per-site tiling: widest x tile that divides Lx (LGF_SITE_TILE overrides, A/B knob)
         int t = (L[0] % 32 == 0) ? 4 : ((L[0] % 16 == 0) ? 1 : 0);
         const char* e = knob("LGF_SITE_TILE");
+#ifdef LGF_DEV_VARIANTS
         if (e && atoi(e) >= 0 && atoi(e) < kNumSiteTiles) t = atoi(e);
+#else
+        if (e && (atoi(e) == 0 || atoi(e) == 1 || atoi(e) == 4)) t = atoi(e);      // tiles 2, 3, 5: -DLGF_DEV_VARIANTS builds only
+#endif
         c->site_tile = t;
         int n = 1;
         for (int i = 0; i < 4; ++i) { c->lo.nb[i] = (L[i] + kSiteTileDims[t][i] - 1) / kSiteTileDims[t][i]; n *= c->lo.nb[i]; }
@@ -1349,6 +1365,24 @@ int lgf_profile_iterate(lgf_ctx* c, int64_t n, double alpha, double ms[5], lgf_r
 }
 
 int64_t lgf_launch_count(const lgf_ctx* c) { return c ? c->launches : 0; }
+
+int lgf_describe(const lgf_ctx* c, char* buf, size_t n) {
+    if (!c || !buf || n == 0) return LGF_EINVAL;
+    const char* fft = c->xy_pipe ? "pipelined (persistent, TMA-fed)" : (c->xy_ct ? "compile-time-sized, one tile per CTA" : "runtime-radix");
+    char k2[96] = "-", k3[96] = "-";
+    if (c->xy_pipe)
+        snprintf(k2, sizeof(k2), "%s x=%dx%d y=%dx%d planes/tile=%d", c->xy_pipe->io ? "fft_xy_pipe_io (TMA-drained)" : "fft_xy_pipe",
+                 c->xy_pipe->x_n1, c->xy_pipe->nx / c->xy_pipe->x_n1, c->xy_pipe->y_n1, c->xy_pipe->ny / c->xy_pipe->y_n1, c->xy_pipe->pb);
+    if (c->zt_pipe)
+        snprintf(k3, sizeof(k3), "%s CX=%d", c->zt_pipe->tstore == 1 ? "fft_zt_pipe3q (quarter ring, TMA tensor stores)" : "fft_zt_pipe / fft_zt_pipe3 (tile ring)",
+                 c->zt_pipe->cx);
+    const char* k5 = c->fused_tile >= 0 ? "k51_update_delta (fused K5+K1)" : (c->site_variant == 2 ? "k5s (shared g)" : (c->site_variant == 1 ? "k5 (thread per site)" : "k5m (thread per site, mu)"));
+    snprintf(buf, n, "lattice %dx%dx%dx%d x %d, %s, %d-real; FFT path: %s; K2: %s; K3: %s; K5: %s; K1 tile %dx%dx%dx%d; %d launches per iteration",
+             c->L[0], c->L[1], c->L[2], c->L[3], c->nbatch, c->precision == LGF_F64 ? "fp64" : "fp32", c->storage, fft, k2, k3, k5,
+             kSiteTileDims[c->site_tile][0], kSiteTileDims[c->site_tile][1], kSiteTileDims[c->site_tile][2], kSiteTileDims[c->site_tile][3],
+             c->launches_per_iter);
+    return LGF_OK;
+}
 
 int lgf_path_info(const lgf_ctx* c, int32_t info[4]) {
     if (!c || !info) return LGF_EINVAL;

@@ -611,3 +611,18 @@ def test_batched_context_fp32_and_limits():
     gb.close()
     assert lgf.workspace_bytes(L, lgf.LGF_F32, lgf.LGF_REAL12, nbatch=4) > 3.9 * lgf.workspace_bytes(L, lgf.LGF_F32, lgf.LGF_REAL12) - (1 << 22)
     assert lgf.workspace_bytes(L, lgf.LGF_F32, lgf.LGF_REAL12, nbatch=5000) == 0      # grid z = nbatch x (z,t) tiles < 2^16
+
+
+def test_describe_reports_the_kernels_a_lattice_fell_onto():
+    U = gi.make_config((8, 8, 64, 64), 95, 0.59)
+    gf = _fixer((8, 8, 64, 64), lgf.LGF_F64, lgf.LGF_REAL12, U)
+    gf.iterate(1, ALPHA)
+    d = gf.describe()
+    assert "pipelined" in d and "fft_zt_pipe3q" in d and "12-real" in d and "fp64" in d and "6 launches" in d
+    gf.close()
+    gf = lgf.GaugeFixer((6, 4, 12, 8))
+    assert "runtime-radix" in gf.describe()                # extents that are not instantiated: the generic kernels, and it says so
+    gf.close()
+    gf = lgf.GaugeFixer((64, 64, 8, 8), lgf.LGF_F32, lgf.LGF_REAL18, nbatch=2)
+    assert "fft_xy_pipe_io" in gf.describe() and "x 2," in gf.describe()
+    gf.close()
