@@ -37,6 +37,7 @@ const ZtPipeEntry* zt_pipe_table_f32(int* n) {
         // the paper's other finite-temperature shapes 48^3 x N_t, N_t = 4, 6, 12
         ZtP3<T, 48, 16, 4, 4, 8, 192, 2, 4>::entry(),
         ZtP3<T, 48, 16, 6, 6, 8, 192, 2, 4>::entry(),
+        ZtP3<T, 48, 16, 12, 12, 8, 128, 2, 3>::entry(),       // 3 x 12 block per thread (36 elements): P2-P4 in one pass
         ZtP<T, 48, 8, 12, 12, 8, 128, 2, 3>::entry(),
         ZtP3Q<T, 64, 16, 64, 4, 4, 512>::entry(),
     };
