@@ -190,6 +190,7 @@ struct lgf_ctx {
     int xyp_grid, ztp_grid;
     alignas(64) CUtensorMap zt_omap;     // fft_zt_pipe3q's output tensor (Delta~, natural layout), stored through the TMA unit
     alignas(64) CUtensorMap xy_bmap;     // fft_xy_pipe_io's output tensor (the layout-B spectrum)
+    alignas(64) CUtensorMap xy_imap;     // fft_xy_inv3's input tensor (Delta~ as planes, box one pad column wider than a plane)
     // fused K5+K1 marching kernel (lgf_site_fused.cuh); -1: not used
     int fused_tile;
     MarchGeom mgeom;
@@ -469,6 +470,17 @@ int make_pipe_maps(lgf_ctx* c) {
         const int rc = encode_map(c, &c->zt_omap, 5, c->ws + c->lo.delta, dims, strides, box);
         if (rc) return rc;
     }
+    if (c->xy_pipe_inv && c->xy_pipe_inv->inv3) {
+        // Delta~ (natural layout) as (2 reals x Nx, Ny, planes); the box is 1 (fp64) / 2 (fp32) columns wider than the plane:
+        // the out-of-range columns are zero-filled and give the shared-memory rows a conflict-free pitch
+        const XyPipeEntry* x = c->xy_pipe_inv;
+        const cuuint64_t nx = c->L[0], ny = c->L[1], pad = c->precision == LGF_F64 ? 1 : 2;
+        const cuuint64_t dims[3] = {2 * nx, ny, (cuuint64_t)c->xyp_args.nplanes};
+        const cuuint64_t strides[2] = {nx * cb, nx * ny * cb};
+        const cuuint32_t box[3] = {(cuuint32_t)(2 * (nx + pad)), (cuuint32_t)ny, (cuuint32_t)x->pb};
+        const int rc = encode_map(c, &c->xy_imap, 3, c->ws + c->lo.delta, dims, strides, box);
+        if (rc) return rc;
+    }
     if (c->xy_pipe->io) {
         const XyPipeArgs& P = c->xyp_args;
         const cuuint64_t dims[4] = {(cuuint64_t)(2 * e->cx), Nz + 1, Nt, (cuuint64_t)(4 * c->nbatch) * P.chunks_per_comp};
@@ -681,7 +693,8 @@ struct Impl {
                 const XyPipeEntry* e = k == 0 ? c->xy_pipe : c->xy_pipe_inv;
                 Cx<T>* inp = k == 0 ? delta_src(c) : dptr;                 // K2 reads Delta where K1 / K51 left it
                 Cx<T>* outp = k == 0 ? d2 : dptr;                          // K2: natural -> layout B; K4: in place
-                void* args[] = {&inp, &outp, &c->xyp_args, &done, &c->xy_bmap};      // (fifth: fft_xy_pipe_io only)
+                void* tmap = (k == 2 && e->inv3) ? (void*)&c->xy_imap : (void*)&c->xy_bmap;      // fifth: fft_xy_inv3 / fft_xy_pipe_io only
+                void* args[] = {&inp, &outp, &c->xyp_args, &done, tmap};
                 CU(launch_exc(c, k == 0 ? e->k_fwd : e->k_inv, dim3(k == 0 ? c->xyp_grid : c->xyp_inv_grid), dim3(e->threads), args, e->smem));
             }
             c->launches++;
@@ -1369,16 +1382,19 @@ int64_t lgf_launch_count(const lgf_ctx* c) { return c ? c->launches : 0; }
 int lgf_describe(const lgf_ctx* c, char* buf, size_t n) {
     if (!c || !buf || n == 0) return LGF_EINVAL;
     const char* fft = c->xy_pipe ? "pipelined (persistent, TMA-fed)" : (c->xy_ct ? "compile-time-sized, one tile per CTA" : "runtime-radix");
-    char k2[96] = "-", k3[96] = "-";
+    char k2[96] = "-", k3[96] = "-", k4[96] = "-";
     if (c->xy_pipe)
         snprintf(k2, sizeof(k2), "%s x=%dx%d y=%dx%d planes/tile=%d", c->xy_pipe->io ? "fft_xy_pipe_io (TMA-drained)" : "fft_xy_pipe",
                  c->xy_pipe->x_n1, c->xy_pipe->nx / c->xy_pipe->x_n1, c->xy_pipe->y_n1, c->xy_pipe->ny / c->xy_pipe->y_n1, c->xy_pipe->pb);
+    if (c->xy_pipe_inv)
+        snprintf(k4, sizeof(k4), "%s planes/tile=%d threads=%d ring=%d", c->xy_pipe_inv->inv3 ? "fft_xy_inv3 (three stages, padded TMA tile)" : "fft_xy_pipe",
+                 c->xy_pipe_inv->pb, c->xy_pipe_inv->threads, c->xy_pipe_inv->nbuf);
     if (c->zt_pipe)
         snprintf(k3, sizeof(k3), "%s CX=%d", c->zt_pipe->tstore == 1 ? "fft_zt_pipe3q (quarter ring, TMA tensor stores)" : "fft_zt_pipe / fft_zt_pipe3 (tile ring)",
                  c->zt_pipe->cx);
     const char* k5 = c->fused_tile >= 0 ? "k51_update_delta (fused K5+K1)" : (c->site_variant == 2 ? "k5s (shared g)" : (c->site_variant == 1 ? "k5 (thread per site)" : "k5m (thread per site, mu)"));
-    snprintf(buf, n, "lattice %dx%dx%dx%d x %d, %s, %d-real; FFT path: %s; K2: %s; K3: %s; K5: %s; K1 tile %dx%dx%dx%d; %d launches per iteration",
-             c->L[0], c->L[1], c->L[2], c->L[3], c->nbatch, c->precision == LGF_F64 ? "fp64" : "fp32", c->storage, fft, k2, k3, k5,
+    snprintf(buf, n, "lattice %dx%dx%dx%d x %d, %s, %d-real; FFT path: %s; K2: %s; K3: %s; K4: %s; K5: %s; K1 tile %dx%dx%dx%d; %d launches per iteration",
+             c->L[0], c->L[1], c->L[2], c->L[3], c->nbatch, c->precision == LGF_F64 ? "fp64" : "fp32", c->storage, fft, k2, k3, k4, k5,
              kSiteTileDims[c->site_tile][0], kSiteTileDims[c->site_tile][1], kSiteTileDims[c->site_tile][2], kSiteTileDims[c->site_tile][3],
              c->launches_per_iter);
     return LGF_OK;

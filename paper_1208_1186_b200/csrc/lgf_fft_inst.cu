@@ -65,30 +65,35 @@ cudaError_t prepare_ct_kernels(int precision) {
 static const XyPipeEntry* xyp_tab(int precision, int* n) { return precision ? xy_pipe_table_f64(n) : xy_pipe_table_f32(n); }
 static const ZtPipeEntry* ztp_tab(int precision, int* n) { return precision ? zt_pipe_table_f64(n) : zt_pipe_table_f32(n); }
 
-// K4 may run on a different tile shape than K2 (both read and write the natural layout on their own):
-// LGF_XYP_INV_VARIANT = v picks the v-th match; default: the same entry as K2 unless a tuned default exists.
+// K4 may run on another entry than K2 as long as the line splits agree (both read and write the natural layout on
+// their own): LGF_XYP_INV_VARIANT = v picks the v-th such entry.
 const XyPipeEntry* find_xy_pipe_inv(int precision, int nx, int ny, const XyPipeEntry* fwd) {
-    const char* e = knob("LGF_XYP_INV_VARIANT");
-    // measured: 48x48 fp32 planes run the inverse pass faster on 1-plane tiles (K4 24.9 -> 22.9 us at 48^3 x 8)
-    int skip = e ? atoi(e) : ((precision == 0 && nx == 48 && ny == 48 && !knob("LGF_XYP_VARIANT")) ? 1 : -1);
-    if (skip < 0 && fwd->k_inv) return fwd;
-    if (skip < 0) skip = 0;                        // a forward-only entry (fft_xy_pipe_io): the first entry that has an inverse kernel
     int n = 0;
     const XyPipeEntry* t = xyp_tab(precision, &n);
-    const XyPipeEntry* last = nullptr;
-    for (int i = 0; i < n; ++i)
-        if (t[i].nx == nx && t[i].ny == ny && t[i].x_n1 == fwd->x_n1 && t[i].y_n1 == fwd->y_n1 && t[i].k_inv) {
-            last = &t[i];
-            if (skip-- == 0) return last;
-        }
-    return last;
+    auto matches = [&](const XyPipeEntry& x) { return x.nx == nx && x.ny == ny && x.x_n1 == fwd->x_n1 && x.y_n1 == fwd->y_n1 && x.k_inv; };
+    if (const char* e = knob("LGF_XYP_INV_VARIANT")) {       // the v-th entry that can invert K2's line splits
+        int skip = atoi(e);
+        const XyPipeEntry* last = nullptr;
+        for (int i = 0; i < n; ++i)
+            if (matches(t[i])) {
+                last = &t[i];
+                if (skip-- == 0) return last;
+            }
+        return last;
+    }
+    for (int i = 0; i < n; ++i)                               // default: the three-stage inverse where one is instantiated,
+        if (matches(t[i]) && t[i].inv3) return &t[i];
+    if (fwd->k_inv) return fwd;                               // else K2's own entry,
+    for (int i = 0; i < n; ++i)                               // else (forward-only K2 entries) the first that fits
+        if (matches(t[i])) return &t[i];
+    return nullptr;
 }
 const XyPipeEntry* find_xy_pipe(int precision, int nx, int ny) {
     int n = 0, skip = variant("LGF_XYP_VARIANT");
     const XyPipeEntry* t = xyp_tab(precision, &n);
     const XyPipeEntry* last = nullptr;
     for (int i = 0; i < n; ++i)
-        if (t[i].nx == nx && t[i].ny == ny) {
+        if (t[i].nx == nx && t[i].ny == ny && t[i].k_fwd) {
             last = &t[i];
             if (skip-- == 0) return last;
         }
@@ -109,7 +114,7 @@ cudaError_t prepare_pipe_kernels(int precision) {
     int n = 0;
     const XyPipeEntry* x = xyp_tab(precision, &n);
     for (int i = 0; i < n; ++i) {
-        cudaError_t e = cudaFuncSetAttribute(x[i].k_fwd, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)x[i].smem);
+        cudaError_t e = x[i].k_fwd ? cudaFuncSetAttribute(x[i].k_fwd, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)x[i].smem) : cudaSuccess;
         if (e == cudaSuccess && x[i].k_inv) e = cudaFuncSetAttribute(x[i].k_inv, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)x[i].smem);
         if (e != cudaSuccess) return e;
     }

@@ -14,14 +14,16 @@ const XyPipeEntry* xy_pipe_table_f64(int* n) {
         XyP<T, 16, 16, 16, 16, 8, 128, 2, 3>::entry(),
         XyP<T, 32, 32, 32, 32, 2, 64, 4, 6>::entry(),
         XyP<T, 32, 32, 32, 32, 4, 128, 2, 3>::entry(),
-        XyP3<T, 48, 4, 48, 12, 2, 192, 2, 3>::entry(),      // K2 in three stages (12*4 x 4*12), K4 in two on the same splits
+        XyP3<T, 48, 4, 48, 12, 2, 192, 2, 3>::entry(),      // K2 in three stages (12*4 x 4*12); its own K4 (two stages): LGF_XYP_INV_VARIANT=0
+        XyInv3<T, 48, 4, 48, 12, 1, 192, 2, 4>::entry(),    // K4: three stages on a padded tile (one round of 192 threads per stage)
         XyP<T, 48, 8, 48, 8, 2, 192, 2, 3>::entry(),     // 576 / 768 items per stage: whole rounds of 192 threads
         XyP<T, 48, 8, 48, 8, 1, 256, 2, 4>::entry(),
         // K2: three stages (16*4 x 4*16), TMA-drained, ONE compute group: with two groups + the I/O warp (17 warps) a
         // scheduler holds five warps, ptxas caps the kernel at 96 registers (104-byte stack frame) and that build failed
         // intermittently on the GPU (5 of 10 bench runs: "unspecified launch failure"); 9 warps leave 170 registers
         XyPIO3<T, 64, 4, 64, 16, 1, 256, 1, 3>::entry(),
-        XyP<T, 64, 4, 64, 16, 1, 256, 2, 3>::entry(),       // its K4
+        XyInv3<T, 64, 4, 64, 16, 1, 256, 1, 3>::entry(),    // its K4: three stages on a padded tile
+        XyP<T, 64, 4, 64, 16, 1, 256, 2, 3>::entry(),       // (K4 in two stages: LGF_XYP_INV_VARIANT=1)
         XyPIO<T, 64, 8, 64, 8, 1, 256, 2, 3>::entry(),      // K2: 32-byte chunks of layout B leave through the TMA unit
         XyP<T, 64, 8, 64, 8, 1, 256, 2, 3>::entry(),        // K4 (and K2 as variant 1)
     };

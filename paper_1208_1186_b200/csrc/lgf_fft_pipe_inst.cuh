@@ -18,6 +18,7 @@ struct XyPipeEntry {
     const void* k_fwd;       // fft_xy_pipe<..., -1, ...>  natural -> layout B
     const void* k_inv;       // fft_xy_pipe<..., +1, ...>  natural -> natural (nullptr: forward-only entry)
     int io;                  // 1: fft_xy_pipe_io (I/O warp, TMA tensor stores into layout B; takes the layout-B CUtensorMap)
+    int inv3;                // 1: inverse-only entry, fft_xy_inv3 (padded TMA tensor load; takes the Delta~ plane CUtensorMap); k_fwd = nullptr
 };
 struct ZtPipeEntry {
     int nz, nt;

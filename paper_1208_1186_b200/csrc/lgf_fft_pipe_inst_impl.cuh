@@ -3,6 +3,7 @@
 #include "lgf_fft_pipe.cuh"
 #include "lgf_fft_pipe3.cuh"
 #include "lgf_fft_pipe_io.cuh"
+#include "lgf_fft_pipe_inv3.cuh"
 #include "lgf_fft_pipe_inst.cuh"
 
 namespace lgf {
@@ -44,6 +45,20 @@ struct XyPIO3 {
     static XyPipeEntry entry() {
         return XyPipeEntry{NX, NY, X1, Y1, PB, GT * NG + 32, NBUF, kSmem,
                            (const void*)&fft_xy_pipe_io<T, SX, SY, -1, PB, GT, NG, NBUF, true>, nullptr, 1};
+    }
+};
+
+// K4 in three register stages on a padded tile (fft_xy_inv3); inverse only: K2 of the lattice is the XyP3 / XyPIO3 entry
+// with the same line splits
+template <typename T, int NX, int X1, int NY, int Y1, int PB, int GT, int NG, int NBUF>
+struct XyInv3 {
+    typedef LineSplit<NX, X1> SX;
+    typedef LineSplit<NY, Y1> SY;
+    static constexpr size_t kSmem = sizeof(Cx<T>) * (size_t)NBUF * PB * (NX + XyPad<T>::value) * NY + 8 * NBUF;
+    static_assert(kSmem <= 227 * 1024, "tile ring exceeds shared memory");
+    static XyPipeEntry entry() {
+        return XyPipeEntry{NX, NY, X1, Y1, PB, GT * NG, NBUF, kSmem, nullptr,
+                           (const void*)&fft_xy_inv3<T, SX, SY, PB, GT, NG, NBUF>, 0, 1};
     }
 };
 
