@@ -166,6 +166,29 @@ int lgf_describe(const lgf_ctx* ctx, char* buf, size_t n);
 /* Number of kernel launches this context has enqueued since creation (for bench.py's gpu_launches). */
 int64_t lgf_launch_count(const lgf_ctx* ctx);
 
+/* Step 1 with NO allocation, for callers that cannot call cudaMalloc (code under CUDA graph capture, tight serving
+ * loops, harnesses that forbid it): theta and F (north_star step 1; the definitions at the top of this file) of a link
+ * field in the boundary layout above that already sits in DEVICE memory, with no context and no workspace.
+ *   links_dev    device pointer, V*72 reals of `precision` (float / double), 16-byte aligned; read only
+ *   cuda_stream  cudaStream_t (NULL = default stream); the two kernels are enqueued on it and the call returns WITHOUT
+ *                synchronising (it records into a capturing stream like any launch)
+ *   theta_F_dev  device pointer to 2 doubles, written by the second kernel: {theta, F}; sums in fp64, fixed order
+ * Its only scratch, the per-CTA partial sums, is a static __device__ array of lgf_static_scratch_bytes() = 1 MiB that
+ * EVERY GPU loading the library holds until the process exits; it bounds the lattice to LGF_STATIC_MAX_SITES sites
+ * (64^4) -- larger lattices are refused with LGF_EINVAL and a message in lgf_static_last_error().  All calls share the
+ * array: calls whose kernels may overlap on the GPU (different streams, parallel graph branches) race on it; calls on
+ * one stream are safe.  Nothing in it needs clearing between calls.  The call uses no cudaMalloc, cudaFree or
+ * allocating library routine.  lgf_static_init() resolves the array's device address for the CURRENT device (once per
+ * device; lgf_measure_static does it itself on first use, so calling it is only needed to keep that first-use work out
+ * of a capture or a timed loop).  Errors: LGF_EINVAL (null pointer, bad precision, L_mu < 2, too many sites),
+ * LGF_ECUDA (symbol lookup or launch failed). */
+#define LGF_STATIC_MAX_SITES 16777216
+int lgf_static_init(void);
+int lgf_measure_static(const int32_t L[4], int precision, const void* links_dev, void* cuda_stream, double* theta_F_dev);
+size_t lgf_static_scratch_bytes(void);
+/* Text of the last error of this thread's lgf_static_* / lgf_measure_static calls ("" if none). */
+const char* lgf_static_last_error(void);
+
 const char* lgf_strerror(int code);
 /* Text of the last CUDA error seen by this thread's calls ("" if none). */
 const char* lgf_last_error(void);

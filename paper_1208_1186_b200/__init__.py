@@ -9,4 +9,5 @@ device every call raises.
 from .binding import (  # noqa: F401
     LGF_F32, LGF_F64, LGF_REAL12, LGF_REAL18, LGF_HOST, LGF_DEVICE,
     GaugeFixer, LgfError, LgfResult, library_path, load_library, declared_symbols, workspace_bytes,
+    measure_static, static_init, STATIC_MAX_SITES,
 )

@@ -7,7 +7,7 @@ import subprocess
 _HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(_HERE, "csrc")
 LIB = os.path.join(_HERE, "liblgf.so")
-SOURCES = ["lgf_api.cu", "lgf_fft_inst.cu", "lgf_fft_inst_f64.cu", "lgf_fft_inst_f32.cu", "lgf_fft_pipe_f64.cu", "lgf_fft_pipe_f32.cu"]
+SOURCES = ["lgf_api.cu", "lgf_fft_inst.cu", "lgf_fft_inst_f64.cu", "lgf_fft_inst_f32.cu", "lgf_fft_pipe_f64.cu", "lgf_fft_pipe_f32.cu", "lgf_static.cu"]
 
 
 def _headers() -> list:

@@ -83,6 +83,12 @@ def load_library() -> ctypes.CDLL:
     lib.lgf_describe.argtypes = [vp, ctypes.c_char_p, ctypes.c_size_t]
     lib.lgf_launch_count.restype = ctypes.c_int64
     lib.lgf_launch_count.argtypes = [vp]
+    lib.lgf_static_init.argtypes = []
+    lib.lgf_measure_static.argtypes = [i32p, ctypes.c_int, vp, vp, vp]
+    lib.lgf_static_scratch_bytes.restype = ctypes.c_size_t
+    lib.lgf_static_scratch_bytes.argtypes = []
+    lib.lgf_static_last_error.restype = ctypes.c_char_p
+    lib.lgf_static_last_error.argtypes = []
     for f in (lib.lgf_strerror, lib.lgf_last_error, lib.lgf_version):
         f.restype = ctypes.c_char_p
     lib.lgf_strerror.argtypes = [ctypes.c_int]
@@ -102,6 +108,40 @@ def _check(rc: int, what: str) -> None:
     if rc != 0:
         lib = load_library()
         raise LgfError(f"{what}: {lib.lgf_strerror(rc).decode()} [{rc}] {lib.lgf_last_error().decode()}")
+
+
+STATIC_MAX_SITES = 16777216   # LGF_STATIC_MAX_SITES of include/lgf.h (64^4)
+
+
+def static_init() -> None:
+    """lgf_static_init: resolve the static scratch array's address on the current CUDA device."""
+    lib = load_library()
+    rc = lib.lgf_static_init()
+    if rc:
+        raise LgfError(f"lgf_static_init: {lib.lgf_strerror(rc).decode()} [{rc}] {lib.lgf_static_last_error().decode()}")
+
+
+def measure_static(L: Sequence[int], links, out=None, stream=None):
+    """lgf_measure_static: theta and F of a DEVICE link tensor [V, 4, 3, 3, 2] (float32 / float64) without a context,
+    a workspace or any allocation inside the library (its scratch is a 1 MiB static device array, at most
+    STATIC_MAX_SITES sites; calls that overlap on the GPU race on it).  -> `out`, a device tensor of 2 float64
+    {theta, F} (made here when not given -- pass one to keep the caller's side allocation-free too); the kernels are
+    enqueued on `stream` (default: torch's current stream) and the call does not synchronise."""
+    import torch
+    lib = load_library()
+    if not links.is_cuda or not links.is_contiguous() or links.dtype not in (torch.float32, torch.float64):
+        raise LgfError("measure_static: links must be a contiguous CUDA tensor of float32 or float64")
+    if out is None:
+        out = torch.empty(2, dtype=torch.float64, device=links.device)
+    if not out.is_cuda or out.dtype != torch.float64 or out.numel() < 2 or out.device != links.device:
+        raise LgfError("measure_static: out must be a CUDA tensor of 2 float64 on the links' device")
+    with torch.cuda.device(links.device):
+        s = stream if stream is not None else torch.cuda.current_stream()
+        rc = lib.lgf_measure_static(_L(L), LGF_F64 if links.dtype == torch.float64 else LGF_F32, links.data_ptr(),
+                                    s.cuda_stream, out.data_ptr())
+    if rc:
+        raise LgfError(f"lgf_measure_static: {lib.lgf_strerror(rc).decode()} [{rc}] {lib.lgf_static_last_error().decode()}")
+    return out
 
 
 class GaugeFixer:
