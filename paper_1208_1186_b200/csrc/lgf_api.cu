@@ -22,6 +22,7 @@
 #include "lgf_site_mu.cuh"
 #include "lgf_site_fused.cuh"
 #include "lgf_wilson.cuh"
+#include "lgf_cluster8.cuh"
 
 using namespace lgf;
 
@@ -195,6 +196,7 @@ struct lgf_ctx {
     int fused_tile;
     MarchGeom mgeom;
     int fused_grid;
+    bool cluster8;               // 8^4, one lattice: lgf_iterate / lgf_fix run k_cluster8_iterate (lgf_cluster8.cuh) instead of the graph
     int cur_host;                // host mirror of DevState::cur
     bool dbg_delta_tilde;        // lgf_debug_get_delta source: Delta~ (after debug_fourier_accelerate) or Delta
     bool loaded, delta_valid;
@@ -755,7 +757,55 @@ struct Impl {
             const int rc = make_pipe_maps(c);
             if (rc) return rc;
         }
+        {
+            const int rc = cluster8_setup(c);
+            if (rc) return rc;
+        }
         return upload_tables<T>(c);
+    }
+    // The single-cluster path (lgf_cluster8.cuh) serves one 8^4 lattice; LGF_CLUSTER=0 (developer knob) keeps the graph path.
+    static int cluster8_setup(lgf_ctx* c) {
+        c->cluster8 = false;
+        const char* off = knob("LGF_CLUSTER");
+        if (c->nbatch != 1 || c->fused_tile >= 0 || (off && atoi(off) == 0)) return LGF_OK;
+        for (int mu = 0; mu < 4; ++mu)
+            if (c->L[mu] != 8) return LGF_OK;
+        const void* k = (const void*)&k_cluster8_iterate<T, NC>;
+        CU(cudaFuncSetAttribute(k, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)Cl8<T, NC>::kSmem));
+        CU(cudaFuncSetAttribute(k, cudaFuncAttributeNonPortableClusterSizeAllowed, 1));
+        cudaLaunchConfig_t cfg = {};
+        cudaLaunchAttribute attr[1];
+        attr[0].id = cudaLaunchAttributeClusterDimension;
+        attr[0].val.clusterDim.x = Cl8<T, NC>::kCtas; attr[0].val.clusterDim.y = 1; attr[0].val.clusterDim.z = 1;
+        cfg.gridDim = dim3(Cl8<T, NC>::kCtas); cfg.blockDim = dim3(Cl8<T, NC>::kThreads);
+        cfg.dynamicSmemBytes = Cl8<T, NC>::kSmem; cfg.attrs = attr; cfg.numAttrs = 1;
+        int nclusters = 0;
+        if (cudaOccupancyMaxActiveClusters(&nclusters, k, &cfg) != cudaSuccess || nclusters < 1) {
+            cudaGetLastError();                // a device that cannot host the 16-CTA cluster keeps the five-kernel graph
+            return LGF_OK;
+        }
+        c->cluster8 = true;
+        return LGF_OK;
+    }
+    // all iterations of one lgf_iterate / lgf_fix call: the kernel reads tol, max_iter and iter from DevState
+    static int cluster8_run(lgf_ctx* c, double alpha) {
+        Cluster8Args a;
+        a.psq = c->ws + c->lo.psq[0];
+        a.scale_num = c->zt_args.scale_num;
+        a.half_alpha = 0.5 * alpha;
+        Cx<T>* U = links(c);
+        Cx<T>* D = delta_src(c);
+        DevState* st = dev_state(c);
+        void* args[] = {&U, &D, &st, &a};
+        cudaLaunchConfig_t cfg = {};
+        cudaLaunchAttribute attr[1];
+        attr[0].id = cudaLaunchAttributeClusterDimension;
+        attr[0].val.clusterDim.x = Cl8<T, NC>::kCtas; attr[0].val.clusterDim.y = 1; attr[0].val.clusterDim.z = 1;
+        cfg.gridDim = dim3(Cl8<T, NC>::kCtas); cfg.blockDim = dim3(Cl8<T, NC>::kThreads);
+        cfg.dynamicSmemBytes = Cl8<T, NC>::kSmem; cfg.stream = c->stream; cfg.attrs = attr; cfg.numAttrs = 1;
+        CU(cudaLaunchKernelExC(&cfg, (const void*)&k_cluster8_iterate<T, NC>, args));
+        c->launches++;
+        return LGF_OK;
     }
     static int load(lgf_ctx* c, const void* src, int memspace) {
         const long long V = c->V;
@@ -1219,6 +1269,15 @@ int lgf_iterate_async(lgf_ctx* c, int64_t n, double alpha) {
     if (!c || n < 0 || !(alpha > 0)) return LGF_EINVAL;
     LGF_NOT_PENDING(c);
     if (!c->loaded) return LGF_ESTATE;
+    if (c->cluster8) {                 // one launch: measure, then n updates with the field resident in the cluster's shared memory
+        int rc8 = init_state(c, -1.0, (long long)n);
+        if (!rc8) rc8 = DISPATCH(c, cluster8_run(c, alpha));
+        if (rc8) return rc8;
+        c->delta_valid = true;
+        c->dbg_delta_tilde = false;
+        c->pending_n = n;
+        return LGF_OK;
+    }
     int rc = ensure_graph(c, alpha);
     if (!rc) rc = init_state(c, -1.0, (long long)n);
     if (!rc && (!c->delta_valid || n == 0)) rc = DISPATCH(c, k1(c, 0));
@@ -1250,6 +1309,18 @@ int lgf_fix(lgf_ctx* c, double alpha, double theta_tol, int64_t max_iter, lgf_re
     if (!c || !out || !(alpha > 0) || max_iter < 0 || !(theta_tol == theta_tol)) return LGF_EINVAL;
     LGF_NOT_PENDING(c);
     if (!c->loaded) return LGF_ESTATE;
+    if (c->cluster8) {                 // the whole convergence loop is one launch (stopping test on the device, every iteration)
+        int rc8 = init_state(c, theta_tol, (long long)max_iter);
+        if (!rc8) rc8 = DISPATCH(c, cluster8_run(c, alpha));
+        if (rc8) return rc8;
+        c->delta_valid = true;
+        c->dbg_delta_tilde = false;
+        lgf_result r8;
+        rc8 = finish(c, &r8, true);
+        if (rc8) return rc8;
+        out[0] = r8;
+        return LGF_OK;
+    }
     int rc = ensure_graph(c, alpha);
     if (!rc) rc = init_state(c, theta_tol, (long long)max_iter);
     if (!rc) rc = DISPATCH(c, k1(c, 0));
@@ -1393,10 +1464,11 @@ int lgf_describe(const lgf_ctx* c, char* buf, size_t n) {
         snprintf(k3, sizeof(k3), "%s CX=%d", c->zt_pipe->tstore == 1 ? "fft_zt_pipe3q (quarter ring, TMA tensor stores)" : "fft_zt_pipe / fft_zt_pipe3 (tile ring)",
                  c->zt_pipe->cx);
     const char* k5 = c->fused_tile >= 0 ? "k51_update_delta (fused K5+K1)" : (c->site_variant == 2 ? "k5s (shared g)" : (c->site_variant == 1 ? "k5 (thread per site)" : "k5m (thread per site, mu)"));
-    snprintf(buf, n, "lattice %dx%dx%dx%d x %d, %s, %d-real; FFT path: %s; K2: %s; K3: %s; K4: %s; K5: %s; K1 tile %dx%dx%dx%d; %d launches per iteration",
+    snprintf(buf, n, "lattice %dx%dx%dx%d x %d, %s, %d-real; FFT path: %s; K2: %s; K3: %s; K4: %s; K5: %s; K1 tile %dx%dx%dx%d; %d launches per iteration%s",
              c->L[0], c->L[1], c->L[2], c->L[3], c->nbatch, c->precision == LGF_F64 ? "fp64" : "fp32", c->storage, fft, k2, k3, k4, k5,
              kSiteTileDims[c->site_tile][0], kSiteTileDims[c->site_tile][1], kSiteTileDims[c->site_tile][2], kSiteTileDims[c->site_tile][3],
-             c->launches_per_iter);
+             c->launches_per_iter,
+             c->cluster8 ? "; lgf_iterate / lgf_fix: k_cluster8_iterate (one launch per call: a 16-CTA cluster holds the field in shared memory)" : "");
     return LGF_OK;
 }
 

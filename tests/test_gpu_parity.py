@@ -561,10 +561,14 @@ def test_wilson_lines_and_singlet_correlator(L):
 
 @pytest.mark.parametrize("L,nbatch", [((8, 8, 8, 8), 5), ((16, 16, 16, 16), 3), ((6, 4, 12, 8), 2), ((16, 16, 8, 8), 4)])
 @pytest.mark.parametrize("prec,stor", MODES)
-def test_batched_context_equals_single_lattice_contexts(L, nbatch, prec, stor):
+def test_batched_context_equals_single_lattice_contexts(monkeypatch, L, nbatch, prec, stor):
     """lgf_create_batch: nbatch different lattices fixed by the same launches.  Each lattice must
     come out exactly as from a context of its own (same kernels, same per-lattice reduction order: bitwise), with its
-    own iteration count -- the lattices converge at different iterations -- and lattice 0 must match the oracle."""
+    own iteration count -- the lattices converge at different iterations -- and lattice 0 must match the oracle.
+    (A single 8^4 lattice would otherwise run the single-cluster kernel, which rounds Delta in another order: the
+    comparison contexts are kept on the five-kernel graph, the kernels the batched context runs.)"""
+    monkeypatch.setenv("LGF_DEVKNOBS", "1")
+    monkeypatch.setenv("LGF_CLUSTER", "0")
     Us = [gi.make_config(L, 80 + b, 0.59 if b % 2 == 0 else 0.57) for b in range(nbatch)]
     stack = torch.cat([gi.as_real(u) for u in Us], 0)
     gb = lgf.GaugeFixer(L, prec, stor, nbatch=nbatch)
@@ -625,4 +629,61 @@ def test_describe_reports_the_kernels_a_lattice_fell_onto():
     gf.close()
     gf = lgf.GaugeFixer((64, 64, 8, 8), lgf.LGF_F32, lgf.LGF_REAL18, nbatch=2)
     assert "fft_xy_pipe_io" in gf.describe() and "x 2," in gf.describe()
+    gf.close()
+
+
+ALL_MODES = [(lgf.LGF_F64, lgf.LGF_REAL18), (lgf.LGF_F64, lgf.LGF_REAL12), (lgf.LGF_F32, lgf.LGF_REAL18), (lgf.LGF_F32, lgf.LGF_REAL12)]
+
+
+@pytest.mark.parametrize("prec,stor", ALL_MODES)
+def test_cluster8_path_against_oracle_and_graph_path(monkeypatch, prec, stor):
+    """8^4 (configs[0]'s shape): lgf_iterate / lgf_fix run the single-cluster kernel (lgf_cluster8.cuh: the field stays
+    in the distributed shared memory of 16 CTAs, one launch per call).  Element by element against the oracle, and
+    against the five-kernel graph path of the same library (LGF_CLUSTER=0); state carries over between calls."""
+    L = (8, 8, 8, 8)
+    U = gi.make_config(L, 23, 0.59)
+    tol_u, tol_rel = (1e-12, 1e-12) if prec == lgf.LGF_F64 else (2e-5, 1e-5)
+    ref, thh, Fh = oracle.iterate(L, U, 6, ALPHA)
+    gf = _fixer(L, prec, stor, U)
+    assert "k_cluster8_iterate" in gf.describe()
+    r0 = gf.iterate(0, ALPHA)                                  # measure only
+    assert r0.iterations == 0 and abs(r0.theta - thh[0]) <= tol_rel * thh[0]
+    r1 = gf.iterate(2, ALPHA)
+    r2 = gf.iterate(4, ALPHA)                                  # 2 + 4 updates in two launches = the oracle's 6
+    assert (r1.iterations, r2.iterations) == (2, 4)
+    got = _cplx(gf.store())
+    assert np.max(np.abs(got - ref)) <= tol_u * 6
+    assert abs(r1.theta - thh[2]) <= 10 * tol_rel * thh[2] and abs(r2.theta - thh[6]) <= 10 * tol_rel * thh[6]
+    assert abs(r2.F - Fh[6]) <= tol_rel * 6
+    rm = gf.measure()                                          # K1 of the five-kernel path on the links the cluster kernel wrote back
+    assert abs(rm.theta - r2.theta) <= (1e-13 if prec == lgf.LGF_F64 else 1e-5) * r2.theta
+    d_cluster = _cplx(gf.debug_delta())
+    gf.close()
+    monkeypatch.setenv("LGF_DEVKNOBS", "1")
+    monkeypatch.setenv("LGF_CLUSTER", "0")
+    gg = _fixer(L, prec, stor, U)
+    assert "k_cluster8_iterate" not in gg.describe()
+    rg = gg.iterate(6, ALPHA)
+    assert np.max(np.abs(_cplx(gg.store()) - got)) <= tol_u
+    assert abs(rg.theta - r2.theta) <= 10 * tol_rel * r2.theta
+    assert np.max(np.abs(_cplx(gg.debug_delta()) - d_cluster)) <= (1e-13 if prec == lgf.LGF_F64 else 2e-5)
+    gg.close()
+
+
+def test_cluster8_fix_counts_iterations_like_the_oracle():
+    """lgf_fix on the cluster path: the stopping test runs on the device after EVERY update; same count as the oracle,
+    0 iterations on a field already below tolerance, max_iter respected."""
+    L = (8, 8, 8, 8)
+    U = gi.make_config(L, 24, 0.59)
+    ref, n, theta, F, thh, Fh = oracle.fix(L, U, ALPHA, 1e-10, 5000)
+    gf = _fixer(L, lgf.LGF_F64, lgf.LGF_REAL12, U)
+    assert "k_cluster8_iterate" in gf.describe()
+    r = gf.fix(ALPHA, 1e-10, 5000)
+    assert r.iterations == n and r.converged and abs(r.theta - theta) <= 1e-9 * theta
+    assert np.max(np.abs(_cplx(gf.store()) - ref)) <= 1e-11
+    again = gf.fix(ALPHA, 1e-10, 5000)                         # already below the tolerance
+    assert again.iterations == 0 and again.converged
+    gf.load(gi.as_real(U, torch.float64))
+    capped = gf.fix(ALPHA, 1e-10, 5)
+    assert capped.iterations == 5 and not capped.converged and abs(capped.theta - thh[5]) <= 1e-11 * thh[5]
     gf.close()
