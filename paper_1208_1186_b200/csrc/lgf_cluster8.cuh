@@ -103,6 +103,19 @@ __device__ __forceinline__ void cl8_line(Cx<T>* f, int stride) {
 
 template <typename T> __device__ __forceinline__ T cl8_shfl(T v, int src) { return __shfl_sync(0xffffffffu, v, src); }
 
+// Cluster barriers.  cg::cluster_group::sync() costs two block barriers, a GPU-scope fence (MEMBAR.ALL.GPU) and an L1
+// invalidate around the hardware barrier.  barrier.cluster counts every thread of every CTA, so the block barriers are
+// redundant; and where the barrier only publishes what the threads of a CTA wrote into their OWN shared memory (the
+// neighbours then read it), a CTA-scope fence + a relaxed arrive is enough: shared memory is the point of coherence
+// for distributed-shared-memory reads.  Where REMOTE stores must have landed (the pushes of step F) the arrive keeps
+// its release semantics.
+__device__ __forceinline__ void cl8_arrive_local() { asm volatile("membar.cta;\n\tbarrier.cluster.arrive.relaxed.aligned;" ::: "memory"); }
+__device__ __forceinline__ void cl8_wait() { asm volatile("barrier.cluster.wait.acquire.aligned;" ::: "memory"); }
+__device__ __forceinline__ void cl8_sync_local() { cl8_arrive_local(); cl8_wait(); }
+__device__ __forceinline__ void cl8_sync_release() {
+    asm volatile("barrier.cluster.arrive.release.aligned;\n\tbarrier.cluster.wait.acquire.aligned;" ::: "memory");
+}
+
 // barrier over the first four warps of the CTA (the 128 threads that run the DFT passes)
 __device__ __forceinline__ void cl8_bar128() { asm volatile("bar.sync 1, 128;" ::: "memory"); }
 
@@ -183,7 +196,7 @@ k_cluster8_iterate(Cx<T>* __restrict__ U, Cx<T>* __restrict__ Dg, DevState* st, 
 #pragma unroll
                     for (int k = 0; k < 6; ++k) gf.m[k] = gsrc[k * 256];
                 } else {
-                    if (mu == 2) cluster.barrier_wait();           // barrier 3 (arrived after step E): the neighbours' g are in place
+                    if (mu == 2) cl8_wait();                        // barrier 3 (arrived after step E): the neighbours' g are in place
                     const uint32_t gsrc = mu == 2 ? G_z : G_t;
 #pragma unroll
                     for (int k = 0; k < 6; ++k) gf.m[k] = cl8_ld(gsrc + (uint32_t)k * 256u * ES, T());
@@ -234,7 +247,7 @@ k_cluster8_iterate(Cx<T>* __restrict__ U, Cx<T>* __restrict__ Dg, DevState* st, 
             }
         }
         CL8_STAMP(11);
-        cluster.sync();                                             // barrier 4: every push has landed
+        cl8_sync_release();                                         // barrier 4: every push has landed
         CL8_STAMP(12);
 #pragma unroll
         for (int b = 0; b < 3; ++b) {
@@ -282,8 +295,17 @@ k_cluster8_iterate(Cx<T>* __restrict__ U, Cx<T>* __restrict__ Dg, DevState* st, 
             cl8_line<-1>(D + 72 * (tid >> 3) + (tid & 7), 9);
         }
         CL8_STAMP(1);
-        cluster.sync();                                             // barrier 1
+        cl8_sync_local();                                           // barrier 1
         CL8_STAMP(2);
+        // ---- B: pull the 16 (z,t) planes of (ky = rank/2; components 2 (rank%2), 2 (rank%2) + 1): the remote loads are
+        //      issued first, the stopping test runs while they are in flight ----
+        const int b_kx = tid & 7, b_zlr = (tid >> 3) & 3, b_cc = (tid >> 5) & 1;
+        Cx<T> pulled[4];
+        {
+            const Cx<T>* src = D + (2 * (rank & 1) + b_cc) * C::kPad + 9 * ((rank >> 1) + 8 * b_zlr) + b_kx;
+#pragma unroll
+            for (int i = 0; i < 4; ++i) pulled[i] = cl8_ld(cl8_map(src, (unsigned)((tid >> 6) + 4 * i)), T());
+        }
         {   // theta, F of the current links: every warp sums the 16 partials with the same butterfly
             const uint32_t p = cl8_map(part, (unsigned)(lane & 15));
             double a = cl8_ld_f64(p), b = cl8_ld_f64(p + 8);
@@ -297,15 +319,10 @@ k_cluster8_iterate(Cx<T>* __restrict__ U, Cx<T>* __restrict__ Dg, DevState* st, 
         }
         if ((theta < tol) || (iter >= max_iter)) break;             // lgf_fix's test (lgf_iterate: tol = -1)
         CL8_STAMP(3);
-        // ---- B: pull the 16 (z,t) planes of (ky = rank/2; components 2 (rank%2), 2 (rank%2) + 1) ----
-        {
-            const int kx = tid & 7, zlr = (tid >> 3) & 3, cc = (tid >> 5) & 1, ky = rank >> 1, c = 2 * (rank & 1) + cc;
-            const Cx<T>* src = D + c * C::kPad + 9 * (ky + 8 * zlr) + kx;
 #pragma unroll
-            for (int i = 0; i < 4; ++i) {
-                const int rr = (tid >> 6) + 4 * i, z = 4 * (rr & 1) + zlr, tt = rr >> 1;
-                Tb[((cc * 8 + tt) * 8 + z) * 8 + kx] = cl8_ld(cl8_map(src, (unsigned)rr), T());
-            }
+        for (int i = 0; i < 4; ++i) {
+            const int rr = (tid >> 6) + 4 * i, z = 4 * (rr & 1) + b_zlr, tt = rr >> 1;
+            Tb[((b_cc * 8 + tt) * 8 + z) * 8 + b_kx] = pulled[i];
         }
         __syncthreads();
         CL8_STAMP(4);
@@ -330,7 +347,7 @@ k_cluster8_iterate(Cx<T>* __restrict__ U, Cx<T>* __restrict__ Dg, DevState* st, 
             cl8_line<+1>(zline, 8);
         }
         CL8_STAMP(5);
-        cluster.sync();                                             // barrier 2
+        cl8_sync_local();                                           // barrier 2
         CL8_STAMP(6);
         // ---- D: pull the spectrum of the own sites back, inverse y, x ----
         {
@@ -355,7 +372,7 @@ k_cluster8_iterate(Cx<T>* __restrict__ U, Cx<T>* __restrict__ Dg, DevState* st, 
         for (int k = 0; k < 6; ++k) G[k * 256 + l] = g.m[k];
         CL8_STAMP(9);
         __syncthreads();                                            // this CTA's g are complete (x, y neighbours; D is free)
-        cluster.barrier_arrive();                                   // barrier 3, waited for inside F before the z, t directions
+        cl8_arrive_local();                                         // barrier 3, waited for inside F before the z, t directions
         CL8_STAMP(10);
         // ---- F, G ----
         update_and_measure(true, g);
