@@ -196,7 +196,7 @@ struct lgf_ctx {
     int fused_tile;
     MarchGeom mgeom;
     int fused_grid;
-    bool cluster8;               // 8^4, one lattice: lgf_iterate / lgf_fix run k_cluster8_iterate (lgf_cluster8.cuh) instead of the graph
+    bool cluster8;               // 8^4 (one cluster per lattice of a batched context): lgf_iterate / lgf_fix run k_cluster8_iterate (lgf_cluster8.cuh) instead of the graph
     int cur_host;                // host mirror of DevState::cur
     bool dbg_delta_tilde;        // lgf_debug_get_delta source: Delta~ (after debug_fourier_accelerate) or Delta
     bool loaded, delta_valid;
@@ -763,11 +763,11 @@ struct Impl {
         }
         return upload_tables<T>(c);
     }
-    // The single-cluster path (lgf_cluster8.cuh) serves one 8^4 lattice; LGF_CLUSTER=0 (developer knob) keeps the graph path.
+    // The single-cluster path (lgf_cluster8.cuh) serves 8^4 lattices (one cluster each); LGF_CLUSTER=0 (developer knob) keeps the graph path.
     static int cluster8_setup(lgf_ctx* c) {
         c->cluster8 = false;
         const char* off = knob("LGF_CLUSTER");
-        if (c->nbatch != 1 || c->fused_tile >= 0 || (off && atoi(off) == 0)) return LGF_OK;
+        if (c->fused_tile >= 0 || (off && atoi(off) == 0)) return LGF_OK;
         for (int mu = 0; mu < 4; ++mu)
             if (c->L[mu] != 8) return LGF_OK;
         const void* k = (const void*)&k_cluster8_iterate<T, NC>;
@@ -801,7 +801,7 @@ struct Impl {
         cudaLaunchAttribute attr[1];
         attr[0].id = cudaLaunchAttributeClusterDimension;
         attr[0].val.clusterDim.x = Cl8<T, NC>::kCtas; attr[0].val.clusterDim.y = 1; attr[0].val.clusterDim.z = 1;
-        cfg.gridDim = dim3(Cl8<T, NC>::kCtas); cfg.blockDim = dim3(Cl8<T, NC>::kThreads);
+        cfg.gridDim = dim3(Cl8<T, NC>::kCtas * c->nbatch); cfg.blockDim = dim3(Cl8<T, NC>::kThreads);
         cfg.dynamicSmemBytes = Cl8<T, NC>::kSmem; cfg.stream = c->stream; cfg.attrs = attr; cfg.numAttrs = 1;
         CU(cudaLaunchKernelExC(&cfg, (const void*)&k_cluster8_iterate<T, NC>, args));
         c->launches++;
@@ -1315,10 +1315,10 @@ int lgf_fix(lgf_ctx* c, double alpha, double theta_tol, int64_t max_iter, lgf_re
         if (rc8) return rc8;
         c->delta_valid = true;
         c->dbg_delta_tilde = false;
-        lgf_result r8;
-        rc8 = finish(c, &r8, true);
+        std::vector<lgf_result> r8((size_t)c->nbatch);
+        rc8 = finish(c, r8.data(), true);
         if (rc8) return rc8;
-        out[0] = r8;
+        for (int b = 0; b < c->nbatch; ++b) out[b] = r8[b];
         return LGF_OK;
     }
     int rc = ensure_graph(c, alpha);

@@ -1,4 +1,5 @@
 // lgf_cluster8.cuh -- the WHOLE iteration loop of an 8^4 lattice in ONE kernel on ONE 16-CTA thread-block cluster
+// (a batched context launches one cluster per lattice)
 // (SURVEY.md §8(f) rank 1 "persistent single-kernel iteration for 8^4"; north_star steps 1-5 and the convergence loop).
 //
 // One lattice of 8^4 is launch-latency-bound on the five-kernel graph (22 us per iteration for 6.8 MB of traffic).
@@ -129,6 +130,12 @@ k_cluster8_iterate(Cx<T>* __restrict__ U, Cx<T>* __restrict__ Dg, DevState* st, 
     constexpr long long V = 4096;
     constexpr int NR = NC / 3;
     constexpr uint32_t ES = sizeof(Cx<T>);
+    {   // batched contexts: one cluster per lattice (the hardware runs as many clusters side by side as it has room for)
+        const int lat = (int)blockIdx.x / C::kCtas;
+        U += (size_t)lat * 4 * NC * V;
+        Dg += (size_t)lat * 4 * V;
+        st += lat;
+    }
 
     Cx<T>* links = reinterpret_cast<Cx<T>*>(cl8_smem);
     Cx<T>* G = links + C::kLinks;

@@ -687,3 +687,39 @@ def test_cluster8_fix_counts_iterations_like_the_oracle():
     capped = gf.fix(ALPHA, 1e-10, 5)
     assert capped.iterations == 5 and not capped.converged and abs(capped.theta - thh[5]) <= 1e-11 * thh[5]
     gf.close()
+
+
+@pytest.mark.parametrize("prec,stor", [(lgf.LGF_F64, lgf.LGF_REAL18), (lgf.LGF_F32, lgf.LGF_REAL12)])
+def test_cluster8_batched_context_runs_one_cluster_per_lattice(prec, stor):
+    """A batched 8^4 context launches one 16-CTA cluster per lattice (more lattices than the GPU hosts clusters at a
+    time: the rest queue).  Every lattice comes out bitwise as from a single-lattice context, with its own iteration
+    count, and lattice 0 matches the oracle."""
+    L, nbatch = (8, 8, 8, 8), 11
+    dt = torch.float64 if prec == lgf.LGF_F64 else torch.float32
+    tol = 1e-10 if prec == lgf.LGF_F64 else 1e-9
+    Us = [gi.make_config(L, 60 + b, 0.59 if b % 2 == 0 else 0.57) for b in range(nbatch)]
+    stack = torch.cat([gi.as_real(u, dt) for u in Us], 0)
+    gb = lgf.GaugeFixer(L, prec, stor, nbatch=nbatch)
+    assert "k_cluster8_iterate" in gb.describe()
+    gb.load(stack)
+    rb = gb.iterate(3, ALPHA)
+    after3 = gb.store().reshape(nbatch, -1, 4, 3, 3, 2)
+    gb.load(stack)
+    rf = gb.fix(ALPHA, tol, 300)
+    fixed = gb.store().reshape(nbatch, -1, 4, 3, 3, 2)
+    assert len({r.iterations for r in rf}) > 1
+    for b in range(nbatch):
+        g1 = _fixer(L, prec, stor, Us[b])
+        r1 = g1.iterate(3, ALPHA)
+        assert (rb[b].theta, rb[b].F, rb[b].iterations) == (r1.theta, r1.F, 3)
+        assert torch.equal(after3[b], g1.store())
+        g1.load(gi.as_real(Us[b], dt))
+        f1 = g1.fix(ALPHA, tol, 300)
+        assert (rf[b].iterations, rf[b].theta, rf[b].F, rf[b].converged) == (f1.iterations, f1.theta, f1.F, f1.converged)
+        assert torch.equal(fixed[b], g1.store())
+        g1.close()
+    if prec == lgf.LGF_F64:
+        ref, n, theta, F, _, _ = oracle.fix(L, Us[0], ALPHA, tol, 300)
+        assert rf[0].iterations == n and abs(rf[0].theta - theta) <= 1e-9 * theta
+        assert np.max(np.abs(_cplx(fixed[0]) - ref)) <= 1e-11
+    gb.close()
