@@ -400,7 +400,8 @@ def main():
                 torch.cuda.synchronize()
                 us = e0.elapsed_time(e1) * 1e3 / 200
                 ent["single" if B == 1 else f"batch_{B}"] = {
-                    "us_per_launch_set": us, "us_per_lattice_iteration": us / B, "lattice_iterations_per_s": B / (us * 1e-6)}
+                    "us_per_launch_set": us, "us_per_lattice_iteration": us / B, "lattice_iterations_per_s": B / (us * 1e-6),
+                    "path": "one 16-CTA cluster per lattice (k_cluster8_iterate)" if "k_cluster8_iterate" in gf.describe() else "launch graph"}
                 gf.close()
                 del gf, Ub
             small[lattice_name(Ls) + " f64_12"] = ent

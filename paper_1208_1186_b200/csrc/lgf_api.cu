@@ -768,6 +768,9 @@ struct Impl {
         c->cluster8 = false;
         const char* off = knob("LGF_CLUSTER");
         if (c->fused_tile >= 0 || (off && atoi(off) == 0)) return LGF_OK;
+        // batched contexts: the B200 hosts 7 fp64 clusters at a time (14 in fp32, two CTAs per SM), a wave of them costs one
+        // lattice's 10 us; past two waves in fp64 the batched launch graph (1.47 us per lattice-iteration) is as fast
+        if (c->precision == LGF_F64 && c->nbatch > 14) return LGF_OK;
         for (int mu = 0; mu < 4; ++mu)
             if (c->L[mu] != 8) return LGF_OK;
         const void* k = (const void*)&k_cluster8_iterate<T, NC>;
