@@ -1461,7 +1461,7 @@ int lgf_describe(const lgf_ctx* c, char* buf, size_t n) {
         snprintf(k2, sizeof(k2), "%s x=%dx%d y=%dx%d planes/tile=%d", c->xy_pipe->io ? "fft_xy_pipe_io (TMA-drained)" : "fft_xy_pipe",
                  c->xy_pipe->x_n1, c->xy_pipe->nx / c->xy_pipe->x_n1, c->xy_pipe->y_n1, c->xy_pipe->ny / c->xy_pipe->y_n1, c->xy_pipe->pb);
     if (c->xy_pipe_inv)
-        snprintf(k4, sizeof(k4), "%s planes/tile=%d threads=%d ring=%d", c->xy_pipe_inv->inv3 ? "fft_xy_inv3 (three stages, padded TMA tile)" : "fft_xy_pipe",
+        snprintf(k4, sizeof(k4), "%s planes/tile=%d threads=%d ring=%d", c->xy_pipe_inv->inv3 ? "fft_xy_inv3 (padded TMA tile, last stage to global)" : "fft_xy_pipe",
                  c->xy_pipe_inv->pb, c->xy_pipe_inv->threads, c->xy_pipe_inv->nbuf);
     if (c->zt_pipe)
         snprintf(k3, sizeof(k3), "%s CX=%d", c->zt_pipe->tstore == 1 ? "fft_zt_pipe3q (quarter ring, TMA tensor stores)" : "fft_zt_pipe / fft_zt_pipe3 (tile ring)",

@@ -14,6 +14,7 @@ const XyPipeEntry* xy_pipe_table_f64(int* n) {
         XyP<T, 16, 16, 16, 16, 8, 128, 2, 3>::entry(),
         XyP<T, 32, 32, 32, 32, 2, 64, 4, 6>::entry(),
         XyP<T, 32, 32, 32, 32, 4, 128, 2, 3>::entry(),
+        XyInv3<T, 32, 32, 32, 32, 2, 64, 3, 6>::entry(),    // K4 at 32 x 32: whole lines on a padded TMA tile, last stage to global
         XyP3<T, 48, 4, 48, 12, 2, 192, 2, 3>::entry(),      // K2 in three stages (12*4 x 4*12); its own K4 (two stages): LGF_XYP_INV_VARIANT=0
         XyInv3<T, 48, 4, 48, 12, 1, 192, 2, 4>::entry(),    // K4: three stages on a padded tile (one round of 192 threads per stage)
         XyP<T, 48, 8, 48, 8, 2, 192, 2, 3>::entry(),     // 576 / 768 items per stage: whole rounds of 192 threads

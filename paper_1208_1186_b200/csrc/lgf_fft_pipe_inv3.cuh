@@ -11,6 +11,8 @@
 // must stay a multiple of 16 bytes, N_x + 2 elements: Q1 alone keeps a 2-way conflict).
 // Shared-memory traffic per plane: the fetch + Q1 (read, write) + Q2 (read, write) + Q3 (read) = 6 traversals
 // instead of 10 for the two-stage kernel (fetch, four passes, copy-out).
+// Lines that fit one thread's registers (32 points, LineSplit<N, N>) run the same scheme in TWO stages: whole x lines in
+// place, whole y lines straight to global memory.
 // Ring of NBUF tile buffers and NG thread groups as in fft_xy_pipe.  Product code (sm_100a); shares nothing with oracle/.
 #pragma once
 #include <cuda.h>
@@ -38,7 +40,8 @@ fft_xy_inv3(const Cx<T>* in, Cx<T>* out, const __grid_constant__ XyPipeArgs A_, 
     if (done && *reinterpret_cast<const volatile int*>(done)) return;
     constexpr int NX = SX::kN, NY = SY::kN, P = NX + XyPad<T>::value, PLANE = P * NY, TILE = PB * PLANE;
     constexpr int A = SY::kN1, B = SY::kN2, C = SX::kN1, D = SX::kN2;
-    static_assert(B > 1 && D > 1 && B * C <= 16, "three-stage K4: the middle block must fit the registers");
+    constexpr bool WHOLE = (B == 1 && D == 1);       // lines that fit one thread's registers (32 points): Q1 and Q3 only
+    static_assert(WHOLE || (B > 1 && D > 1 && B * C <= 16), "three-stage K4: the middle block must fit the registers");
     static_assert((TILE * sizeof(Cx<T>)) % 128 == 0 && (P * sizeof(Cx<T>)) % 16 == 0, "tensor-load alignment");
     // NBUF % NG == 0: a buffer is always re-armed by the group that consumes it.  With NG = 2, NBUF = 3 (the groups hand
     // buffers to each other, as fft_xy_pipe does without trouble) this kernel ended in "unspecified launch failure" on
@@ -73,6 +76,29 @@ fft_xy_inv3(const Cx<T>* in, Cx<T>* out, const __grid_constant__ XyPipeArgs A_, 
         const int nvalid = min(PB, A_.nplanes - plane0);
         mbar_wait(&full[buf], (uint32_t)((i / NBUF) & 1));
 
+        if constexpr (WHOLE) {
+            // ---- whole x lines in place (lanes along y: the odd pitch keeps them conflict-free) ----
+            for (int it = gtid; it < PB * NY; it += GT) {
+                Cx<T>* s = tile + (it / NY) * PLANE + (it % NY) * P;
+                Cx<T> v[NX];
+                static_for<0, NX>([&](auto j) { v[j.value] = s[j.value]; });
+                RegFft<NX, +1, T>::run(v);
+                static_for<0, NX>([&](auto j) { s[j.value] = v[j.value]; });
+            }
+            group_sync<GT, NG>(g);
+            // ---- whole y lines, straight to global memory (lanes along x: coalesced) ----
+            for (int it = gtid; it < PB * NX; it += GT) {
+                const int x = it % NX, pl = it / NX;
+                if (pl < nvalid) {
+                    const Cx<T>* s = tile + pl * PLANE + x;
+                    Cx<T> v[NY];
+                    static_for<0, NY>([&](auto k) { v[k.value] = s[k.value * P]; });
+                    RegFft<NY, +1, T>::run(v);
+                    Cx<T>* gp = out + (size_t)(plane0 + pl) * (NX * NY) + x;
+                    static_for<0, NY>([&](auto k) { st_cx_keep(gp + (size_t)k.value * NX, v[k.value], keep); });
+                }
+            }
+        } else {
         // ---- Q1: x, 16-point stage (lanes along y) ----
         for (int it = gtid; it < PB * NY * C; it += GT) {
             const int y = it % NY, k1x = (it / NY) % C, pl = it / (NY * C);
@@ -113,6 +139,7 @@ fft_xy_inv3(const Cx<T>* in, Cx<T>* out, const __grid_constant__ XyPipeArgs A_, 
                 Cx<T>* gp = out + (size_t)(plane0 + pl) * (NX * NY) + (size_t)n2y * NX + x;
                 static_for<0, A>([&](auto m) { st_cx_keep(gp + (size_t)m.value * B * NX, v[m.value], keep); });
             }
+        }
         }
         // ---- hand the buffer back to the TMA unit for tile i + NBUF ----
         fence_proxy_async();
