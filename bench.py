@@ -342,8 +342,11 @@ def main():
         host_in = gi.as_real(U, dt).cpu().pin_memory()
         host_out = torch.empty_like(host_in).pin_memory()
         gf = lgf.GaugeFixer(L, lgf.LGF_F64 if prec == "f64" else lgf.LGF_F32, stor, device=str(dev))
+        # untimed warm-up of the same three calls (first launches load their kernels lazily)
         gf.load(host_in)
         gf.iterate(W, ALPHA)
+        gf.fix(ALPHA, 1e-15, W)
+        gf.store(host_out)
         barrier()
         t0 = time.perf_counter()
         gf.load(host_in)

@@ -93,7 +93,7 @@ bool factor23(int n, Axis* ax) {
 }
 
 struct Layout {          // byte offsets into the workspace
-    size_t state, partials, tw[4], twi[4], psq[4], links, links_bytes, delta, delta2, delta3, staging, total;
+    size_t state, partials, tw[4], twi[4], psq[4], links, links_bytes, delta, delta2, delta3, staging, staging_bytes, total;
     int nblocks_site;
     int nb[4];
     int nblocks_mu;          // tiling of the (site, direction) kernels
@@ -146,7 +146,8 @@ Layout make_layout(const int32_t L[4], int precision, int storage, bool fused, i
     lo.delta2 = off; off += align_up(B * 4 * (V / L[2]) * (size_t)(L[2] + 1) * 2 * w);
     lo.delta3 = off; off += fused ? align_up(B * 4 * V * 2 * w) : 0;   // Delta of the new links (fused path: K1/K51 out, K2 in)
     const size_t stage_sites = V < (size_t)kStageSites ? V : (size_t)kStageSites;
-    lo.staging = off; off += align_up(stage_sites * 36 * 2 * w);
+    lo.staging_bytes = align_up(stage_sites * 36 * 2 * w);          // two buffers: the copy of one chunk runs beside the transpose of the other
+    lo.staging = off; off += 2 * lo.staging_bytes;
     lo.total = off;
     return lo;
 }
@@ -217,6 +218,10 @@ struct lgf_ctx {
     // of a batch; LGF_DEFER_FINISH=0 puts it back behind K1
     bool defer_finish;
     cudaStream_t fin_stream;
+    // lgf_load / lgf_store from / to HOST memory: the PCIe copies run on io_stream beside the layout transposes on the context's
+    // stream, through two staging buffers (io_copied[b]: the copy into / out of buffer b is done; io_moved[b]: its transpose is)
+    cudaStream_t io_stream;
+    cudaEvent_t io_start, io_copied[2], io_moved[2];
     cudaEvent_t ev_fork, ev_join;
     bool pdl_enabled, pdl;
     int pdl_mask, pdl_idx;       // which launches of the body (bit i: i-th launch) carry the attribute
@@ -529,7 +534,7 @@ struct Impl {
     static Cx<T>* delta(lgf_ctx* c) { return reinterpret_cast<Cx<T>*>(c->ws + c->lo.delta); }      // Delta~ (natural)
     // where K1 / K51 write Delta of the current links and K2 reads it
     static Cx<T>* delta_src(lgf_ctx* c) { return reinterpret_cast<Cx<T>*>(c->ws + (c->fused_tile >= 0 ? c->lo.delta3 : c->lo.delta)); }
-    static Cx<T>* staging(lgf_ctx* c) { return reinterpret_cast<Cx<T>*>(c->ws + c->lo.staging); }
+    static Cx<T>* staging(lgf_ctx* c, int which = 0) { return reinterpret_cast<Cx<T>*>(c->ws + c->lo.staging + (size_t)which * c->lo.staging_bytes); }
 
     static int k1(lgf_ctx* c, int mode, bool with_finish = true) {
         double2* partials = reinterpret_cast<double2*>(c->ws + c->lo.partials);
@@ -817,6 +822,11 @@ struct Impl {
         reset_cur_kernel<<<1, c->nbatch, 0, c->stream>>>(dev_state(c));
         c->launches++;
         CU(cudaGetLastError());
+        int k = 0;                                         // staging chunks so far (all lattices of a batched context)
+        if (memspace != LGF_DEVICE) {
+            CU(cudaEventRecord(c->io_start, c->stream));   // whatever produced `src` on this stream comes first
+            CU(cudaStreamWaitEvent(c->io_stream, c->io_start, 0));
+        }
         for (int b = 0; b < c->nbatch; ++b) {             // the lattices of a batched context lie back to back, here and there
             Cx<T>* Ub = links(c) + (size_t)b * 4 * NC * V;
             const Cx<T>* sb = reinterpret_cast<const Cx<T>*>(src) + (size_t)b * V * 36;
@@ -826,13 +836,19 @@ struct Impl {
                 c->launches++;
                 CU(cudaGetLastError());
             } else {
-                for (long long s0 = 0; s0 < V; s0 += kStageSites) {
+                // chunk k is copied into staging buffer k % 2 on io_stream while chunk k - 1 is transposed on the context's stream
+                for (long long s0 = 0; s0 < V; s0 += kStageSites, ++k) {
                     const long long ns = (V - s0 < kStageSites) ? V - s0 : kStageSites;
-                    CU(cudaMemcpyAsync(staging(c), sb + (size_t)s0 * 36, (size_t)ns * 36 * sizeof(Cx<T>), cudaMemcpyHostToDevice, c->stream));
+                    const int buf = k & 1;
+                    if (k >= 2) CU(cudaStreamWaitEvent(c->io_stream, c->io_moved[buf], 0));      // its previous contents are consumed
+                    CU(cudaMemcpyAsync(staging(c, buf), sb + (size_t)s0 * 36, (size_t)ns * 36 * sizeof(Cx<T>), cudaMemcpyHostToDevice, c->io_stream));
+                    CU(cudaEventRecord(c->io_copied[buf], c->io_stream));
+                    CU(cudaStreamWaitEvent(c->stream, c->io_copied[buf], 0));
                     const long long n = ns * 36;
-                    aos_to_soa<T, NC><<<(unsigned)((n + thr - 1) / thr), thr, 0, c->stream>>>(staging(c), Ub, V, s0, ns);
+                    aos_to_soa<T, NC><<<(unsigned)((n + thr - 1) / thr), thr, 0, c->stream>>>(staging(c, buf), Ub, V, s0, ns);
                     c->launches++;
                     CU(cudaGetLastError());
+                    CU(cudaEventRecord(c->io_moved[buf], c->stream));
                 }
             }
         }
@@ -842,6 +858,7 @@ struct Impl {
     static int store(lgf_ctx* c, void* dst, int memspace) {
         const long long V = c->V;
         const int thr = 256;
+        int k = 0;                                         // staging chunks so far (all lattices of a batched context)
         for (int b = 0; b < c->nbatch; ++b) {
             const Cx<T>* Ub = links(c) + (size_t)b * 4 * NC * V;
             Cx<T>* db = reinterpret_cast<Cx<T>*>(dst) + (size_t)b * V * 36;
@@ -851,16 +868,23 @@ struct Impl {
                 c->launches++;
                 CU(cudaGetLastError());
             } else {
-                for (long long s0 = 0; s0 < V; s0 += kStageSites) {
+                // chunk k is transposed into staging buffer k % 2 on the context's stream while chunk k - 1 leaves on io_stream
+                for (long long s0 = 0; s0 < V; s0 += kStageSites, ++k) {
                     const long long ns = (V - s0 < kStageSites) ? V - s0 : kStageSites;
                     const long long n = ns * 4;
-                    soa_to_aos<T, NC><<<(unsigned)((n + thr - 1) / thr), thr, 0, c->stream>>>(Ub, staging(c), V, s0, ns);
+                    const int buf = k & 1;
+                    if (k >= 2) CU(cudaStreamWaitEvent(c->stream, c->io_copied[buf], 0));        // its previous contents have left
+                    soa_to_aos<T, NC><<<(unsigned)((n + thr - 1) / thr), thr, 0, c->stream>>>(Ub, staging(c, buf), V, s0, ns);
                     c->launches++;
                     CU(cudaGetLastError());
-                    CU(cudaMemcpyAsync(db + (size_t)s0 * 36, staging(c), (size_t)ns * 36 * sizeof(Cx<T>), cudaMemcpyDeviceToHost, c->stream));
+                    CU(cudaEventRecord(c->io_moved[buf], c->stream));
+                    CU(cudaStreamWaitEvent(c->io_stream, c->io_moved[buf], 0));
+                    CU(cudaMemcpyAsync(db + (size_t)s0 * 36, staging(c, buf), (size_t)ns * 36 * sizeof(Cx<T>), cudaMemcpyDeviceToHost, c->io_stream));
+                    CU(cudaEventRecord(c->io_copied[buf], c->io_stream));
                 }
             }
         }
+        if (memspace != LGF_DEVICE) CU(cudaStreamSynchronize(c->io_stream));
         CU(cudaStreamSynchronize(c->stream));
         return LGF_OK;
     }
@@ -1141,6 +1165,15 @@ static int create_common(const int32_t L[4], int precision, int storage, int nba
         if (ce == cudaSuccess) ce = cudaEventCreateWithFlags(&c->ev_join, cudaEventDisableTiming);
         if (ce != cudaSuccess) rc = cuda_fail(ce, "deferred-finish stream/events");
     }
+    if (!rc) {
+        cudaError_t ce = cudaStreamCreateWithFlags(&c->io_stream, cudaStreamNonBlocking);
+        if (ce == cudaSuccess) ce = cudaEventCreateWithFlags(&c->io_start, cudaEventDisableTiming);
+        for (int i = 0; i < 2 && ce == cudaSuccess; ++i) {
+            ce = cudaEventCreateWithFlags(&c->io_copied[i], cudaEventDisableTiming);
+            if (ce == cudaSuccess) ce = cudaEventCreateWithFlags(&c->io_moved[i], cudaEventDisableTiming);
+        }
+        if (ce != cudaSuccess) rc = cuda_fail(ce, "boundary copy stream/events");
+    }
     for (int i = 0; i < 2 && !rc; ++i) {
         cudaError_t e = cudaEventCreateWithFlags(&c->ev[i], cudaEventDisableTiming);
         if (e != cudaSuccess) rc = cuda_fail(e, "cudaEventCreate");
@@ -1209,6 +1242,12 @@ int lgf_destroy(lgf_ctx* c) {
     if (c->fin_stream) cudaStreamDestroy(c->fin_stream);
     if (c->ev_fork) cudaEventDestroy(c->ev_fork);
     if (c->ev_join) cudaEventDestroy(c->ev_join);
+    if (c->io_stream) { cudaStreamSynchronize(c->io_stream); cudaStreamDestroy(c->io_stream); }
+    if (c->io_start) cudaEventDestroy(c->io_start);
+    for (int i = 0; i < 2; ++i) {
+        if (c->io_copied[i]) cudaEventDestroy(c->io_copied[i]);
+        if (c->io_moved[i]) cudaEventDestroy(c->io_moved[i]);
+    }
     for (int i = 0; i < 2; ++i)
         if (c->ev[i]) cudaEventDestroy(c->ev[i]);
     if (c->host_state) cudaFreeHost(c->host_state);
