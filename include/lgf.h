@@ -112,7 +112,9 @@ int lgf_store(lgf_ctx* ctx, void* links, int memspace);
 int lgf_measure(lgf_ctx* ctx, lgf_result* out);
 
 /* Exactly n updates (steps 2-5, then step 1 on the new links), no stopping test.  n >= 0, alpha > 0.
- * One host synchronisation at the end. */
+ * One host synchronisation at the end.  (Which kernels run is the library's choice and lgf_describe reports it: most
+ * lattices replay a five-kernel CUDA graph per update; an 8^4 lattice runs the whole call as ONE kernel on a 16-CTA
+ * thread-block cluster that keeps the field in distributed shared memory.  Results agree to rounding.) */
 int lgf_iterate(lgf_ctx* ctx, int64_t n, double alpha, lgf_result* out);
 
 /* Same as lgf_iterate but only enqueues the work on the context's stream and returns; the result
